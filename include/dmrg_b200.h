@@ -1,0 +1,219 @@
+/* dmrg_b200.h -- C ABI of the B200-native DMRG hot path (arXiv:1309.5571).
+ *
+ * The path: the superblock projection  X' = H_SB X  inside the Davidson iteration
+ * (Alg. 3).  With U(1) sectors the projection is the list of dense
+ * block products
+ *        X'_jl += c_alpha * A_{alpha,i->j} X_ik B_{alpha,k->l}^T        (Eq. 11)
+ * over the operator pairs of the LR strategy (Eq. 9-10), plus the
+ * BLAS-2 part of Alg. 3 (lines 3, 5, 12, 13; Alg. 4).
+ *
+ * Conventions
+ *  - Every function returns int: 0 = DMRG_OK, >0 informational, <0 error.  No exception
+ *    crosses the ABI; dmrg_last_error() gives the text of the last error of a handle
+ *    (or of plan creation when the handle is NULL).
+ *  - "DEVICE" pointers are CUDA device pointers owned by the caller; "HOST" pointers are
+ *    host memory read (or written) during the call only.  The library never frees caller
+ *    memory.  All device work is enqueued on the `cuda_stream` argument (a cudaStream_t
+ *    passed as void*; NULL = the legacy default stream).
+ *  - Flat superblock vector (readings A1, A5):
+ *    the target sector is the concatenation, over the admissible sector pairs (i,k) with
+ *    label(i) + label(k) == target sorted by (left sector index, right sector index), of
+ *    the row-major d_i x d_k segment X_ik (left index slow, right index fast -- the
+ *    memory order of the composite index of A (x) B).  dmrg_get_layout() reports it.
+ *  - Operators are lists of dense row-major blocks A_{src->dst} of shape
+ *    dims[dst] x dims[src].  The label shift of an operator is read off
+ *    its blocks, never assumed (reading A4).
+ *  - FP64 throughout.  Results are run-to-run bitwise reproducible: no floating-point
+ *    atomics, every reduction has a fixed order (reading A23).
+ */
+#ifndef DMRG_B200_H
+#define DMRG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------------------ */
+#define DMRG_OK               0
+#define DMRG_NOT_CONVERGED    1   /* dmrg_lowest_eigenpair: max_iter applies spent        */
+#define DMRG_E_INVALID_ARG   (-1)
+#define DMRG_E_SECTOR        (-2) /* empty target space; block dims disagree with sector
+                                     dims; blocks of one operator with different shifts  */
+#define DMRG_E_ALLOC         (-3)
+#define DMRG_E_CUDA          (-4)
+#define DMRG_E_NUMERIC       (-5) /* NaN / zero norm (Davidson breakdown)                */
+
+#define DMRG_HEISENBERG 1         /* PAPER.md:L43-54, Eq. 1-3                            */
+#define DMRG_HUBBARD    2         /* PAPER.md:L66-82, Eq. 4-8 (spin-1/2)                 */
+
+/* ---- problem statement ------------------------------------------------------------- */
+
+/* Quantum-number sectors of one (enlarged) block. HOST arrays. */
+typedef struct {
+    int32_t        n_labels;   /* 1 = S_z (any integer unit); 2 = (N_up, N_dn)            */
+    int32_t        n_sectors;
+    const int32_t *labels;     /* HOST [n_sectors][n_labels]                              */
+    const int32_t *dims;       /* HOST [n_sectors], >= 0 (0 = empty sector, skipped, A26) */
+} dmrg_sectors;
+
+/* One sector-blocked operator.  Index arrays HOST, data DEVICE. */
+typedef struct {
+    int32_t        n_blocks;   /* 0 = operator absent                                     */
+    const int32_t *src;        /* HOST [n_blocks]: block b maps sector src[b] ...         */
+    const int32_t *dst;        /* HOST [n_blocks]: ... to sector dst[b]                   */
+    const int64_t *offset;     /* HOST [n_blocks]: element offset of block b in data      */
+    const int32_t *ld;         /* HOST [n_blocks]: row stride (>= dims[src[b]]), row-major */
+    const double  *data;       /* DEVICE                                                  */
+} dmrg_block_op;
+
+/* The superblock in the LR strategy.  Terms (reading A3):
+ *  Heisenberg: H_L(x)I + I(x)H_R + J/2 (S+_L(x)S-_R + S-_L(x)S+_R) + J*Delta Sz_L(x)Sz_R
+ *  Hubbard:    H_L(x)I + I(x)H_R - t sum_sigma [ (c+_L,s P_L)(x)c_R,s + (P_L c_L,s)(x)c+_R,s ]
+ *              + U (D_L(x)I + I(x)D_R),  P_L = (-1)^{N_L} (reading A6: the fermion string of a
+ *              right-block operator runs over the whole left block).
+ *  S- and c are the transposes of the S+ and c+ blocks given here. */
+typedef struct {
+    int32_t       model;                      /* DMRG_HEISENBERG | DMRG_HUBBARD          */
+    double        J, Delta, t, U;
+    dmrg_sectors  left, right;
+    dmrg_block_op H_L, H_R;                   /* block-diagonal, symmetric               */
+    dmrg_block_op Sz_L, Sp_L, Sz_R, Sp_R;     /* Heisenberg boundary-site operators      */
+    dmrg_block_op Cup_L, Cdn_L, Cup_R, Cdn_R; /* Hubbard c+_sigma of the boundary site,
+                                                 strings inside the own block only       */
+    dmrg_block_op D_L, D_R;                   /* optional sum_j n_up n_dn of the block;
+                                                 folded into H_L/H_R at plan time (A7)   */
+    const int32_t *target;                    /* HOST [n_labels]                         */
+} dmrg_problem;
+
+typedef struct {
+    int32_t  k_max;     /* Davidson basis limit, 2..32 (PAPER.md:L271 uses 20)           */
+    double   tol;       /* ||r||_2 <= tol, absolute (reading A17)                        */
+    int32_t  max_iter;  /* cap on H applies in dmrg_lowest_eigenpair                     */
+    int32_t  reorth;    /* classical Gram-Schmidt passes in lines 12-13: 1 or 2 (A16)    */
+    uint64_t seed;      /* start vector seed when x0 == NULL                             */
+    int32_t  tile;      /* projection tile selector: 0 = auto                            */
+    int32_t  check_every; /* dmrg_lowest_eigenpair: host reads the device convergence flag
+                             every this many iterations (0 = default 8)                   */
+} dmrg_options;
+
+typedef struct {
+    int64_t n;                 /* target-sector dimension                                 */
+    int32_t n_pairs;           /* admissible sector pairs (segments)                      */
+    int32_t n_records;         /* operation records                       */
+    int32_t n_gemms;           /* dense GEMMs per apply (identity factors skipped)        */
+    int64_t flop_per_apply;    /* algorithmic FLOP, reading A24                           */
+    int64_t operator_elems;    /* operator-block elements the apply reads (unpadded)      */
+    int64_t apply_bytes;       /* 8*(operator_elems + 2n): compulsory traffic per apply   */
+    int32_t stage1_units, stage2_units; /* CTAs of the two grouped launches               */
+    int32_t stage2_split_tiles;/* output tiles whose concatenated K is split              */
+    int64_t pool_bytes;        /* repacked operator pool                                  */
+    int64_t workspace_bytes;   /* T + split-K partials + Davidson scratch                 */
+    int64_t device_bytes;      /* everything the plan allocated on the device             */
+    int32_t kernel_launches_per_apply;
+    int32_t kernel_launches_per_step;  /* dmrg_davidson_step at reorth passes = options   */
+} dmrg_stats;
+
+typedef struct dmrg_plan *dmrg_handle_t;
+
+/* ---- plan -------------------------------------------------------------------------- */
+
+/* Builds everything that is constant over the Davidson iterations ("A, B
+ * are fixed"): admissible pairs, operation records grouped by output segment (L342, L358:
+ * "all records of the same output on the same [owner]" -> atomics-free accumulation),
+ * per-record association order by FLOP (A24), the repacked operator pool (scaled,
+ * transposed, 16-byte aligned rows), work units for the two grouped launches, diag(H_SB)
+ * (A14) and all workspaces.  Reads the operator data on the device (stream NULL) and
+ * synchronises before returning.  opts may be NULL (k_max 20, tol 1e-10, max_iter 2000,
+ * reorth 1).  On failure *out = NULL and dmrg_last_error(NULL) has the reason. */
+int dmrg_plan_create(const dmrg_problem *problem, const dmrg_options *opts, dmrg_handle_t *out);
+int dmrg_plan_destroy(dmrg_handle_t h);
+
+/* Flat-vector layout.  Any output pointer may be NULL.  left_sector/right_sector/seg_offset
+ * are HOST arrays of n_pairs entries (call once with NULL arrays to get n_pairs). */
+int dmrg_get_layout(dmrg_handle_t h, int64_t *n, int32_t *n_pairs,
+                    int32_t *left_sector, int32_t *right_sector, int64_t *seg_offset);
+int dmrg_get_stats(dmrg_handle_t h, dmrg_stats *stats);
+/* diag(H_SB) on the target sector (reading A14) copied to a DEVICE array of n doubles. */
+int dmrg_get_diag(dmrg_handle_t h, double *d_out, void *cuda_stream);
+const char *dmrg_last_error(dmrg_handle_t h);
+
+/* ---- hot path ---------------------------------------------------------------------- */
+
+/* y = H_SB x on the target sector: Eq. 11 over all records (Alg. 3 line 2).
+ * x, y DEVICE, n doubles each, must not overlap; y is overwritten.  Asynchronous on the
+ * stream; no allocation; two kernel launches. */
+int dmrg_apply_H(dmrg_handle_t h, const double *x, double *y, void *cuda_stream);
+
+/* Starts a Davidson run (Alg. 3 "Require"): V(:,0) = x0/||x0||, k = 1,
+ * B = 0.  V, W DEVICE, column-contiguous n x k_max with column stride ldv >= n doubles
+ * (ldv even keeps 16-byte vector loads).  x0 DEVICE n doubles, or NULL for a seeded
+ * N(0,1)-like start (options.seed; reading A19).  start_at_argmin_diag != 0 with
+ * x0 == NULL selects the deterministic start e_argmin(D) (lowest index on ties). */
+int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag,
+                       double *V, double *W, int64_t ldv, void *cuda_stream);
+
+/* One call of Alg. 3 (readings A13-A18):
+ *   W(:,k-1) = H_SB V(:,k-1); B(0:k,k-1) = V^T W(:,k-1); (lambda,y) lowest eigenpair of B;
+ *   x = V y; r = W y - lambda x; rho = ||r||; if rho <= tol -> converged;
+ *   restart collapse when k == k_max (A15); t = r / g(lambda - D) (A14);
+ *   reorth x { s = V^T t; t -= V s } (A16); V(:,k) = t/||t||; k += 1.
+ * In: *k = number of orthonormal columns held in V (W(:,0..k-2) = H V(:,0..k-2), B as
+ * left by the previous call).  Out: *k updated (k+1, or 2 after a restart; unchanged when
+ * converged), *lambda, *resnorm, *converged (HOST).  Synchronises the stream once to read
+ * these three numbers.  Returns DMRG_E_NUMERIC on breakdown (A18/step 9). */
+int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k,
+                       double *lambda, double *resnorm, int32_t *converged, void *cuda_stream);
+
+/* Small-matrix state of the last step for lock-step tests: B (k_max x k_max, row-major)
+ * and y (k_max) copied to HOST arrays (either may be NULL).  dmrg_set_small loads B
+ * (e.g. to resume from a caller-kept state). */
+int dmrg_get_small(dmrg_handle_t h, double *B_host, double *y_host, void *cuda_stream);
+int dmrg_set_small(dmrg_handle_t h, const double *B_host, void *cuda_stream);
+
+/* x_out = V y / ||V y|| with the y of the last step (Alg. 3 line 5/8). DEVICE n doubles. */
+int dmrg_ritz_vector(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
+                     double *x_out, void *cuda_stream);
+
+/* Driver (Alg. 3 looped): lowest eigenpair of H_SB on the target sector.
+ * x0 DEVICE or NULL (seeded start; start_at_argmin_diag as in dmrg_davidson_init);
+ * x_out DEVICE n doubles (normalised Ritz vector); lambda, resnorm, iters HOST.
+ * Uses plan-owned V, W (allocated on first use: 2 * n * k_max doubles).  The convergence
+ * test runs on the device; the host polls it every options.check_every iterations, so up
+ * to check_every-1 no-op launches may follow convergence; the reported iteration count is
+ * the exact one.  Returns DMRG_OK, DMRG_NOT_CONVERGED or an error. */
+int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag,
+                          double *x_out, double *lambda, double *resnorm, int32_t *iters,
+                          void *cuda_stream);
+
+/* ---- the Davidson BLAS-2 kernels on their own (Alg. 3 lines 3, 5-6, 12-13; Alg. 4) --- */
+
+/* out[0..k) = V(:,0..k)^T w   (gemv_trans).  out DEVICE k doubles. */
+int dmrg_gemv_trans(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
+                    const double *w, double *out, void *cuda_stream);
+/* t -= V(:,0..k) s  and  *nrm2_out = ||t||^2 (gemv). s, nrm2_out DEVICE. */
+int dmrg_gemv_sub(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
+                  const double *s, double *t, double *nrm2_out, void *cuda_stream);
+
+/* ---- measurement helpers ----------------------------------------------------------- */
+
+/* Register-only issue-rate probes used as the FP64 roofline denominator (MEASURED_PEAKS.json
+ * has no FP64 entry): kind 0 = DFMA, 1 = DMMA.8x8x4 (mma.sync m8n8k4 f64).  Runs `reps`
+ * launches on the stream, returns the best TFLOP/s in *tflops (HOST). */
+int dmrg_probe_fp64_peak(int32_t kind, int32_t reps, double *tflops, void *cuda_stream);
+/* Streams `bytes` of device memory (read-only sum) and returns GB/s (HOST). */
+int dmrg_probe_hbm_read(int64_t bytes, int32_t reps, double *gbs, void *cuda_stream);
+/* Per-kernel device time of the last dmrg_davidson_step when timing was enabled with
+ * dmrg_set_timing(h, 1): ms[0] apply stage 1, [1] apply stage 2, [2] V^T w, [3] small eig,
+ * [4] residual+precondition, [5] orthogonalise (all passes), [6] normalise/append,
+ * [7] restart collapse.  HOST array of 8. */
+int dmrg_set_timing(dmrg_handle_t h, int32_t enable);
+int dmrg_get_timing(dmrg_handle_t h, double *ms8);
+
+int dmrg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMRG_B200_H */

@@ -1,0 +1,364 @@
+"""Thin ctypes binding of libdmrg_b200.so (include/dmrg_b200.h) -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the library; PyTorch is used for device
+memory (``torch.empty(..., device='cuda')``), ``data_ptr()`` and the current stream.  There is
+no CPU fallback: importing works without a GPU (so the symbol table can be checked), but every
+compute call needs the built library and a CUDA device and fails loudly otherwise.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmrg_b200.so")
+
+DMRG_OK, DMRG_NOT_CONVERGED = 0, 1
+DMRG_E_INVALID_ARG, DMRG_E_SECTOR, DMRG_E_ALLOC, DMRG_E_CUDA, DMRG_E_NUMERIC = -1, -2, -3, -4, -5
+DMRG_HEISENBERG, DMRG_HUBBARD = 1, 2
+
+EXPORTS = [
+    "dmrg_plan_create", "dmrg_plan_destroy", "dmrg_get_layout", "dmrg_get_stats", "dmrg_get_diag",
+    "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_get_small",
+    "dmrg_set_small", "dmrg_ritz_vector", "dmrg_lowest_eigenpair", "dmrg_gemv_trans", "dmrg_gemv_sub",
+    "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_version",
+]
+
+
+class DmrgError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dmrg_b200 error {code}: {msg}")
+        self.code = code
+
+
+class _Sectors(C.Structure):
+    _fields_ = [("n_labels", C.c_int32), ("n_sectors", C.c_int32),
+                ("labels", C.POINTER(C.c_int32)), ("dims", C.POINTER(C.c_int32))]
+
+
+class _BlockOp(C.Structure):
+    _fields_ = [("n_blocks", C.c_int32), ("src", C.POINTER(C.c_int32)), ("dst", C.POINTER(C.c_int32)),
+                ("offset", C.POINTER(C.c_int64)), ("ld", C.POINTER(C.c_int32)), ("data", C.c_void_p)]
+
+
+_OP_NAMES = ["H_L", "H_R", "Sz_L", "Sp_L", "Sz_R", "Sp_R", "Cup_L", "Cdn_L", "Cup_R", "Cdn_R", "D_L", "D_R"]
+
+
+class _Problem(C.Structure):
+    _fields_ = ([("model", C.c_int32), ("J", C.c_double), ("Delta", C.c_double), ("t", C.c_double),
+                 ("U", C.c_double), ("left", _Sectors), ("right", _Sectors)]
+                + [(nm, _BlockOp) for nm in _OP_NAMES] + [("target", C.POINTER(C.c_int32))])
+
+
+class _Options(C.Structure):
+    _fields_ = [("k_max", C.c_int32), ("tol", C.c_double), ("max_iter", C.c_int32), ("reorth", C.c_int32),
+                ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n_pairs", C.c_int32), ("n_records", C.c_int32), ("n_gemms", C.c_int32),
+                ("flop_per_apply", C.c_int64), ("operator_elems", C.c_int64), ("apply_bytes", C.c_int64),
+                ("stage1_units", C.c_int32), ("stage2_units", C.c_int32), ("stage2_split_tiles", C.c_int32),
+                ("pool_bytes", C.c_int64), ("workspace_bytes", C.c_int64), ("device_bytes", C.c_int64),
+                ("kernel_launches_per_apply", C.c_int32), ("kernel_launches_per_step", C.c_int32)]
+
+    def as_dict(self):
+        return {f: getattr(self, f) for f, _ in self._fields_}
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the C-ABI library and declare the signatures.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1309_5571_b200.build` "
+                          "(nvcc, sm_100a).  There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    pi32, pi64, pdbl = C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)
+    sig = {
+        "dmrg_plan_create": [C.POINTER(_Problem), C.POINTER(_Options), C.POINTER(vp)],
+        "dmrg_plan_destroy": [vp],
+        "dmrg_get_layout": [vp, pi64, pi32, pi32, pi32, pi64],
+        "dmrg_get_stats": [vp, C.POINTER(Stats)],
+        "dmrg_get_diag": [vp, vp, vp],
+        "dmrg_apply_H": [vp, vp, vp, vp],
+        "dmrg_davidson_init": [vp, vp, i32, vp, vp, i64, vp],
+        "dmrg_davidson_step": [vp, vp, vp, i64, pi32, pdbl, pdbl, pi32, vp],
+        "dmrg_get_small": [vp, pdbl, pdbl, vp],
+        "dmrg_set_small": [vp, pdbl, vp],
+        "dmrg_ritz_vector": [vp, vp, i64, i32, vp, vp],
+        "dmrg_lowest_eigenpair": [vp, vp, i32, vp, pdbl, pdbl, pi32, vp],
+        "dmrg_gemv_trans": [vp, vp, i64, i32, vp, vp, vp],
+        "dmrg_gemv_sub": [vp, vp, i64, i32, vp, vp, vp, vp],
+        "dmrg_probe_fp64_peak": [i32, i32, pdbl, vp],
+        "dmrg_probe_hbm_read": [i64, i32, pdbl, vp],
+        "dmrg_set_timing": [vp, i32],
+        "dmrg_get_timing": [vp, pdbl],
+        "dmrg_version": [],
+    }
+    for name, args in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = args
+        fn.restype = C.c_int
+    lib.dmrg_last_error.argtypes = [vp]
+    lib.dmrg_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1309_5571_b200 needs a CUDA device (B200, sm_100a); there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(stream=None) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _ptr(t) -> int:
+    return 0 if t is None else int(t.data_ptr())
+
+
+def _check_vec(t, n: int, name: str):
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name}: need a contiguous float64 CUDA tensor")
+    if t.numel() < n:
+        raise ValueError(f"{name}: needs at least {n} elements")
+
+
+class Plan:
+    """Owns a dmrg_handle_t plus the device copies of the operator blocks."""
+
+    def __init__(self, problem, k_max: int = 20, tol: float = 1e-10, max_iter: int = 2000, reorth: int = 1,
+                 seed: int = 1, check_every: int = 8, device: Optional[str] = None):
+        torch = _torch()
+        self._lib = load_library()
+        self._keep = []
+        self.device = torch.device(device or "cuda:0")
+        torch.cuda.set_device(self.device)
+        pr = _Problem()
+        model = problem.model
+        pr.model = {"heisenberg": DMRG_HEISENBERG, "hubbard": DMRG_HUBBARD}.get(model, model)
+        pr.J, pr.Delta, pr.t, pr.U = float(problem.J), float(problem.Delta), float(problem.t), float(problem.U)
+        pr.left = self._sectors(problem.left)
+        pr.right = self._sectors(problem.right)
+        for nm in _OP_NAMES:
+            setattr(pr, nm, self._block_op(problem.ops.get(nm)))
+        tgt = np.ascontiguousarray(np.asarray(problem.target, dtype=np.int32).ravel())
+        self._keep.append(tgt)
+        pr.target = tgt.ctypes.data_as(C.POINTER(C.c_int32))
+        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every))
+        h = C.c_void_p()
+        rc = self._lib.dmrg_plan_create(C.byref(pr), C.byref(opt), C.byref(h))
+        if rc != DMRG_OK:
+            raise DmrgError(rc, (self._lib.dmrg_last_error(None) or b"").decode())
+        self._h = h
+        self.k_max = int(k_max)
+        n, npairs = C.c_int64(), C.c_int32()
+        self._lib.dmrg_get_layout(self._h, C.byref(n), C.byref(npairs), None, None, None)
+        self.n, self.n_pairs = int(n.value), int(npairs.value)
+        ls = np.zeros(self.n_pairs, np.int32); rs = np.zeros(self.n_pairs, np.int32); off = np.zeros(self.n_pairs, np.int64)
+        self._lib.dmrg_get_layout(self._h, None, None, ls.ctypes.data_as(C.POINTER(C.c_int32)),
+                                  rs.ctypes.data_as(C.POINTER(C.c_int32)), off.ctypes.data_as(C.POINTER(C.c_int64)))
+        self.left_sector, self.right_sector, self.seg_offset = ls, rs, off
+
+    # ---- marshalling helpers
+    def _sectors(self, s) -> _Sectors:
+        labels = np.ascontiguousarray(np.asarray(s.labels, dtype=np.int32).reshape(len(s.dims), -1))
+        dims = np.ascontiguousarray(np.asarray(s.dims, dtype=np.int32))
+        self._keep += [labels, dims]
+        return _Sectors(labels.shape[1], dims.shape[0], labels.ctypes.data_as(C.POINTER(C.c_int32)),
+                        dims.ctypes.data_as(C.POINTER(C.c_int32)))
+
+    def _block_op(self, op) -> _BlockOp:
+        torch = _torch()
+        if op is None or len(op.blocks) == 0:
+            return _BlockOp(0, None, None, None, None, None)
+        src = np.ascontiguousarray(np.asarray(op.src, dtype=np.int32))
+        dst = np.ascontiguousarray(np.asarray(op.dst, dtype=np.int32))
+        sizes = np.array([b.size for b in op.blocks], dtype=np.int64)
+        offset = np.ascontiguousarray(np.concatenate([[0], np.cumsum(sizes)[:-1]]).astype(np.int64))
+        ld = np.ascontiguousarray(np.array([b.shape[1] for b in op.blocks], dtype=np.int32))
+        flat = np.concatenate([np.ascontiguousarray(b, dtype=np.float64).ravel() for b in op.blocks]) \
+            if sizes.sum() > 0 else np.zeros(1)
+        data = torch.from_numpy(flat).to(self.device)
+        self._keep += [src, dst, offset, ld, data]
+        ip = C.POINTER(C.c_int32)
+        return _BlockOp(len(op.blocks), src.ctypes.data_as(ip), dst.ctypes.data_as(ip),
+                        offset.ctypes.data_as(C.POINTER(C.c_int64)), ld.ctypes.data_as(ip), C.c_void_p(data.data_ptr()))
+
+    def _check(self, rc: int):
+        if rc < 0:
+            raise DmrgError(rc, (self._lib.dmrg_last_error(self._h) or b"").decode())
+        return rc
+
+    # ---- plan queries
+    def stats(self) -> dict:
+        s = Stats()
+        self._check(self._lib.dmrg_get_stats(self._h, C.byref(s)))
+        return s.as_dict()
+
+    def diag(self):
+        torch = _torch()
+        d = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        self._check(self._lib.dmrg_get_diag(self._h, _ptr(d), _stream_ptr()))
+        return d
+
+    def new_basis(self, ldv: Optional[int] = None):
+        """Allocates V, W as (k_max, ldv) row-major tensors = column-contiguous n x k_max."""
+        torch = _torch()
+        ldv = int(ldv) if ldv is not None else (self.n + 15) // 16 * 16
+        V = torch.zeros((self.k_max, ldv), dtype=torch.float64, device=self.device)
+        W = torch.zeros((self.k_max, ldv), dtype=torch.float64, device=self.device)
+        return V, W
+
+    # ---- hot path (same names as the C entry points, without the prefix)
+    def apply_H(self, x, y=None, stream=None):
+        torch = _torch()
+        _check_vec(x, self.n, "x")
+        if y is None:
+            y = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        _check_vec(y, self.n, "y")
+        self._check(self._lib.dmrg_apply_H(self._h, _ptr(x), _ptr(y), _stream_ptr(stream)))
+        return y
+
+    def davidson_init(self, V, W, x0=None, start_at_argmin_diag: bool = False, stream=None):
+        if x0 is not None:
+            _check_vec(x0, self.n, "x0")
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_davidson_init(self._h, _ptr(x0), int(bool(start_at_argmin_diag)), _ptr(V), _ptr(W),
+                                                 int(ldv), _stream_ptr(stream)))
+
+    def davidson_step(self, V, W, k: int, stream=None) -> Tuple[int, float, float, bool]:
+        kk, lam, rho, conv = C.c_int32(int(k)), C.c_double(), C.c_double(), C.c_int32()
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_davidson_step(self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), C.byref(lam),
+                                                 C.byref(rho), C.byref(conv), _stream_ptr(stream)))
+        return int(kk.value), float(lam.value), float(rho.value), bool(conv.value)
+
+    def get_small(self):
+        B = np.zeros((self.k_max, self.k_max)); y = np.zeros(self.k_max)
+        pd = C.POINTER(C.c_double)
+        self._check(self._lib.dmrg_get_small(self._h, B.ctypes.data_as(pd), y.ctypes.data_as(pd), _stream_ptr()))
+        return B, y
+
+    def set_small(self, B):
+        B = np.ascontiguousarray(B, dtype=np.float64)
+        assert B.shape == (self.k_max, self.k_max)
+        self._check(self._lib.dmrg_set_small(self._h, B.ctypes.data_as(C.POINTER(C.c_double)), _stream_ptr()))
+
+    def ritz_vector(self, V, k: int, stream=None):
+        torch = _torch()
+        x = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_ritz_vector(self._h, _ptr(V), int(ldv), int(k), _ptr(x), _stream_ptr(stream)))
+        return x
+
+    def lowest_eigenpair(self, x0=None, start_at_argmin_diag: bool = False, x_out=None, stream=None):
+        """Returns (rc, lambda, x, resnorm, iters); rc is DMRG_OK or DMRG_NOT_CONVERGED."""
+        torch = _torch()
+        if x0 is not None:
+            _check_vec(x0, self.n, "x0")
+        if x_out is None:
+            x_out = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        lam, rho, it = C.c_double(), C.c_double(), C.c_int32()
+        rc = self._check(self._lib.dmrg_lowest_eigenpair(self._h, _ptr(x0), int(bool(start_at_argmin_diag)), _ptr(x_out),
+                                                         C.byref(lam), C.byref(rho), C.byref(it), _stream_ptr(stream)))
+        return rc, float(lam.value), x_out, float(rho.value), int(it.value)
+
+    def gemv_trans(self, V, k: int, w, out=None, stream=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty(k, dtype=torch.float64, device=self.device)
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_gemv_trans(self._h, _ptr(V), int(ldv), int(k), _ptr(w), _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def gemv_sub(self, V, k: int, s, t, nrm2=None, stream=None):
+        torch = _torch()
+        if nrm2 is None:
+            nrm2 = torch.empty(1, dtype=torch.float64, device=self.device)
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_gemv_sub(self._h, _ptr(V), int(ldv), int(k), _ptr(s), _ptr(t), _ptr(nrm2), _stream_ptr(stream)))
+        return nrm2
+
+    # ---- host-buffer entry (end-to-end measurement: H2D of x, apply, D2H of y)
+    def apply_H_host(self, x_host, y_host, x_dev=None, y_dev=None, stream=None):
+        """x_host, y_host: pinned CPU float64 tensors of n elements.  Copies x to the device, applies H
+        through the C ABI and copies y back on the same stream; synchronises before returning."""
+        torch = _torch()
+        if x_dev is None:
+            x_dev = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        if y_dev is None:
+            y_dev = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        x_dev.copy_(x_host, non_blocking=True)
+        self.apply_H(x_dev, y_dev, stream)
+        y_host.copy_(y_dev, non_blocking=True)
+        (stream or torch.cuda.current_stream()).synchronize()
+        return y_host
+
+    def set_timing(self, enable: bool):
+        self._check(self._lib.dmrg_set_timing(self._h, int(bool(enable))))
+
+    def get_timing(self):
+        ms = np.zeros(8)
+        self._check(self._lib.dmrg_get_timing(self._h, ms.ctypes.data_as(C.POINTER(C.c_double))))
+        return ms
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.dmrg_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ---- module-level functions with the names of the C entry points ---------------------------
+def dmrg_plan_create(problem, **opts) -> Plan:
+    return Plan(problem, **opts)
+
+
+def dmrg_apply_H(plan: Plan, x, y=None, stream=None):
+    return plan.apply_H(x, y, stream)
+
+
+def dmrg_davidson_step(plan: Plan, V, W, k: int, stream=None):
+    return plan.davidson_step(V, W, k, stream)
+
+
+def dmrg_lowest_eigenpair(plan: Plan, x0=None, start_at_argmin_diag: bool = False, x_out=None, stream=None):
+    return plan.lowest_eigenpair(x0, start_at_argmin_diag, x_out, stream)
+
+
+def dmrg_probe_fp64_peak(kind: int = 1, reps: int = 3) -> float:
+    lib = load_library(); _torch()
+    v = C.c_double()
+    rc = lib.dmrg_probe_fp64_peak(int(kind), int(reps), C.byref(v), _stream_ptr())
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return float(v.value)
+
+
+def dmrg_probe_hbm_read(nbytes: int = 1 << 31, reps: int = 3) -> float:
+    lib = load_library(); _torch()
+    v = C.c_double()
+    rc = lib.dmrg_probe_hbm_read(int(nbytes), int(reps), C.byref(v), _stream_ptr())
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return float(v.value)

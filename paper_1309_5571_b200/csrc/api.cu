@@ -1,0 +1,240 @@
+// api.cu -- the extern "C" surface declared in include/dmrg_b200.h.  Argument checking and
+// marshalling only; every step of the path runs in the kernels of gemm.cu / davidson.cu.
+#include <cmath>
+#include <cstring>
+#include "internal.h"
+
+namespace dmrg { const std::string &global_error(); }
+using namespace dmrg;
+
+namespace {
+inline Plan *P(dmrg_handle_t h) { return reinterpret_cast<Plan *>(h); }
+inline cudaStream_t S(void *s) { return reinterpret_cast<cudaStream_t>(s); }
+
+int read_state(Plan *p, cudaStream_t st) {
+    cudaError_t e = cudaMemcpyAsync(p->state_host, p->state, sizeof(DavState), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, std::string("state read-back: ") + cudaGetErrorString(e));
+    return DMRG_OK;
+}
+void ensure_timing(Plan *p) {
+    if (!p->timing.created) {
+        for (auto &e : p->timing.ev) cudaEventCreate(&e);
+        p->timing.created = true;
+    }
+}
+}  // namespace
+
+extern "C" {
+
+int dmrg_version(void) { return 100; }
+
+const char *dmrg_last_error(dmrg_handle_t h) {
+    if (h) return P(h)->err.c_str();
+    return global_error().c_str();
+}
+
+int dmrg_plan_create(const dmrg_problem *problem, const dmrg_options *opts, dmrg_handle_t *out) {
+    if (!out) return fail(nullptr, DMRG_E_INVALID_ARG, "out is NULL");
+    Plan *p = nullptr;
+    int rc = plan_build(problem, opts, &p);
+    *out = reinterpret_cast<dmrg_handle_t>(p);
+    return rc;
+}
+
+int dmrg_plan_destroy(dmrg_handle_t h) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    cudaDeviceSynchronize();
+    plan_free(P(h));
+    return DMRG_OK;
+}
+
+int dmrg_get_layout(dmrg_handle_t h, int64_t *n, int32_t *n_pairs, int32_t *left_sector, int32_t *right_sector,
+                    int64_t *seg_offset) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (n) *n = p->n;
+    if (n_pairs) *n_pairs = (int32_t)p->pairL.size();
+    for (size_t q = 0; q < p->pairL.size(); q++) {
+        if (left_sector) left_sector[q] = p->pairL[q];
+        if (right_sector) right_sector[q] = p->pairR[q];
+        if (seg_offset) seg_offset[q] = p->segOff[q];
+    }
+    return DMRG_OK;
+}
+
+int dmrg_get_stats(dmrg_handle_t h, dmrg_stats *stats) {
+    if (!h || !stats) return DMRG_E_INVALID_ARG;
+    P(h)->stats.device_bytes = P(h)->device_bytes;
+    *stats = P(h)->stats;
+    return DMRG_OK;
+}
+
+int dmrg_get_diag(dmrg_handle_t h, double *d_out, void *stream) {
+    if (!h || !d_out) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    cudaError_t e = cudaMemcpyAsync(d_out, p->D, sizeof(double) * p->n, cudaMemcpyDeviceToDevice, S(stream));
+    return e == cudaSuccess ? DMRG_OK : fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+}
+
+int dmrg_apply_H(dmrg_handle_t h, const double *x, double *y, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!x || !y) return fail(p, DMRG_E_INVALID_ARG, "apply_H: NULL vector");
+    if ((x <= y && y < x + p->n) || (y <= x && x < y + p->n)) return fail(p, DMRG_E_INVALID_ARG, "apply_H: x and y overlap");
+    return apply_H(p, x, y, nullptr, S(stream));
+}
+
+int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag, double *V, double *W,
+                       int64_t ldv, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "davidson_init: NULL basis or ldv < n");
+    return dav_init(p, x0, start_at_argmin_diag, V, W, ldv, S(stream));
+}
+
+int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, double *lambda,
+                       double *resnorm, int32_t *converged, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step: NULL argument");
+    if (p->timing.enabled) ensure_timing(p);
+    int k_next = *k;
+    int rc = dav_enqueue_step(p, V, W, ldv, *k, S(stream), &k_next);
+    if (rc != DMRG_OK) return rc;
+    rc = read_state(p, S(stream));
+    if (rc != DMRG_OK) return rc;
+    const DavState &st = *p->state_host;
+    if (lambda) *lambda = st.lambda;
+    if (resnorm) *resnorm = st.rho;
+    if (converged) *converged = (st.done == 1) ? 1 : 0;
+    if (st.error || st.done == 2) return fail(p, DMRG_E_NUMERIC, "Davidson breakdown: zero or non-finite norm");
+    if (st.done != 1) *k = k_next;
+    if (p->timing.enabled) {
+        for (int q = 0; q < 8; q++) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, p->timing.ev[q], p->timing.ev[q + 1]);
+            p->timing.ms[q] = ms;
+        }
+    }
+    return DMRG_OK;
+}
+
+int dmrg_get_small(dmrg_handle_t h, double *B_host, double *y_host, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    int rc = read_state(p, S(stream));
+    if (rc != DMRG_OK) return rc;
+    if (B_host) {
+        const int km = p->opt.k_max;
+        for (int i = 0; i < km; i++) for (int j = 0; j < km; j++) B_host[i * km + j] = p->state_host->B[i * KMAX + j];
+    }
+    if (y_host) for (int i = 0; i < p->opt.k_max; i++) y_host[i] = p->state_host->y[i];
+    return DMRG_OK;
+}
+
+int dmrg_set_small(dmrg_handle_t h, const double *B_host, void *stream) {
+    if (!h || !B_host) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    int rc = read_state(p, S(stream));
+    if (rc != DMRG_OK) return rc;
+    const int km = p->opt.k_max;
+    memset(p->state_host->B, 0, sizeof(p->state_host->B));
+    for (int i = 0; i < km; i++) for (int j = 0; j < km; j++) p->state_host->B[i * KMAX + j] = B_host[i * km + j];
+    cudaError_t e = cudaMemcpyAsync(p->state->B, p->state_host->B, sizeof(p->state_host->B), cudaMemcpyHostToDevice, S(stream));
+    if (e == cudaSuccess) e = cudaStreamSynchronize(S(stream));
+    return e == cudaSuccess ? DMRG_OK : fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+}
+
+int dmrg_ritz_vector(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, double *x_out, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !x_out || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "ritz_vector: bad argument");
+    return dav_ritz(p, V, ldv, k, x_out, S(stream));
+}
+
+int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag, double *x_out,
+                          double *lambda, double *resnorm, int32_t *iters, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!x_out) return fail(p, DMRG_E_INVALID_ARG, "lowest_eigenpair: x_out is NULL");
+    cudaStream_t st = S(stream);
+    const int k_max = p->opt.k_max;
+    if (!p->Vown) {
+        p->ldv_own = (p->n + 15) / 16 * 16;
+        size_t bytes = sizeof(double) * (size_t)p->ldv_own * k_max;
+        if (cudaMalloc((void **)&p->Vown, bytes) != cudaSuccess || cudaMalloc((void **)&p->Wown, bytes) != cudaSuccess) {
+            cudaFree(p->Vown); p->Vown = nullptr; p->Wown = nullptr; cudaGetLastError();
+            return fail(p, DMRG_E_ALLOC, "lowest_eigenpair: cannot allocate the Davidson basis");
+        }
+        p->device_bytes += 2 * (long long)bytes;
+    }
+    const bool was_timing = p->timing.enabled;
+    p->timing.enabled = false;
+    int rc = dav_init(p, x0, start_at_argmin_diag, p->Vown, p->Wown, p->ldv_own, st);
+    int k = 1, done = 0;
+    for (int it = 1; rc == DMRG_OK && it <= p->opt.max_iter; it++) {
+        int k_next = k;
+        rc = dav_enqueue_step(p, p->Vown, p->Wown, p->ldv_own, k, st, &k_next);
+        if (rc != DMRG_OK) break;
+        k = k_next;
+        if (it % p->opt.check_every == 0 || it == p->opt.max_iter) {
+            rc = read_state(p, st);
+            if (rc != DMRG_OK) break;
+            done = p->state_host->done;
+            if (done) break;
+        }
+    }
+    p->timing.enabled = was_timing;
+    if (rc != DMRG_OK) return rc;
+    const DavState &s = *p->state_host;
+    if (lambda) *lambda = s.lambda;
+    if (resnorm) *resnorm = s.rho;
+    if (iters) *iters = s.iters;
+    if (s.error || done == 2) return fail(p, DMRG_E_NUMERIC, "Davidson breakdown: zero or non-finite norm");
+    // Ritz vector of the last executed step; after a restart step V(:,0) already is x/||x||
+    if (done != 1 && s.k_used == k_max)
+        cudaMemcpyAsync(x_out, p->Vown, sizeof(double) * p->n, cudaMemcpyDeviceToDevice, st);
+    else
+        rc = dav_ritz(p, p->Vown, p->ldv_own, s.k_used, x_out, st);
+    if (rc != DMRG_OK) return rc;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    return done == 1 ? DMRG_OK : DMRG_NOT_CONVERGED;
+}
+
+int dmrg_gemv_trans(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, const double *w, double *out, void *stream) {
+    if (!h || !V || !w || !out) return DMRG_E_INVALID_ARG;
+    return dav_gemv_trans(P(h), V, ldv, k, w, out, S(stream));
+}
+
+int dmrg_gemv_sub(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, const double *s, double *t,
+                  double *nrm2_out, void *stream) {
+    if (!h || !V || !s || !t || !nrm2_out) return DMRG_E_INVALID_ARG;
+    return dav_gemv_sub(P(h), V, ldv, k, s, t, nrm2_out, S(stream));
+}
+
+int dmrg_probe_fp64_peak(int32_t kind, int32_t reps, double *tflops, void *stream) {
+    if (!tflops || reps < 1 || kind < 0 || kind > 1) return DMRG_E_INVALID_ARG;
+    return probe_fp64(kind, reps, tflops, S(stream));
+}
+
+int dmrg_probe_hbm_read(int64_t bytes, int32_t reps, double *gbs, void *stream) {
+    if (!gbs || reps < 1) return DMRG_E_INVALID_ARG;
+    return probe_hbm(bytes, reps, gbs, S(stream));
+}
+
+int dmrg_set_timing(dmrg_handle_t h, int32_t enable) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    P(h)->timing.enabled = enable != 0;
+    if (enable) ensure_timing(P(h));
+    return DMRG_OK;
+}
+
+int dmrg_get_timing(dmrg_handle_t h, double *ms8) {
+    if (!h || !ms8) return DMRG_E_INVALID_ARG;
+    for (int q = 0; q < 8; q++) ms8[q] = P(h)->timing.ms[q];
+    return DMRG_OK;
+}
+
+}  // extern "C"

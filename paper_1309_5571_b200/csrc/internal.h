@@ -1,0 +1,133 @@
+// internal.h -- structures shared by the host planner and the sm_100a kernels.
+// Not part of the ABI (include/dmrg_b200.h is).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+#include <cuda_runtime.h>
+#include "../../include/dmrg_b200.h"
+
+namespace dmrg {
+
+// ---- grouped GEMM descriptors (projection, Eq. 11; L340 operation records) ----
+// Every product on the path is brought to the form  C(MxN) = sum_items P(MxK) * Q(KxN), all
+// row-major: right-block factors are stored transposed (B^T) and left-block factors pre-scaled
+// by the record coefficient at plan time (operators are constant over the iteration, L340).
+enum Base : uint8_t { BASE_X = 0, BASE_Y = 1, BASE_T = 2, BASE_POOL = 3, BASE_PART = 4, BASE_COUNT = 5 };
+
+struct GemmItem {
+    long long p_off, q_off;   // element offsets in their bases
+    int ldp, ldq, K;
+    uint8_t p_base, q_base;
+    uint8_t p_vec2, q_vec2;   // 16-byte loads legal (even offset, even ld)
+};
+
+struct GemmUnit {
+    long long c_off;          // C(0,0) in its base
+    long long part_off;       // first split-K partial slot of this tile (elements, BASE_PART)
+    int ldc, M, N;            // whole output matrix
+    int m0, n0;               // tile origin
+    int item_begin, item_count;
+    int kt_begin, kt_count;   // range in the flattened k-tile sequence of the tile's items
+    int tile_id;              // split-K counter index (-1: not split)
+    int split_idx, n_split;
+    uint8_t c_base, c_vec2;
+    uint8_t pad[2];
+};
+
+struct BasePtrs { double *p[BASE_COUNT]; };
+
+// tile shape of the grouped kernel (gemm.cu is compiled for exactly these)
+constexpr int BM = 64, BN = 64, BK = 16;
+
+// ---- plan-time device jobs ----
+struct RepackJob {            // dst(rows x cols, ld) = s1*op(src1) + s2*op(src2), op = transpose if flag
+    const double *src1, *src2;
+    long long dst_off;
+    int ld1, ld2, ldd, rows, cols;   // rows/cols of dst
+    int transpose;
+    double s1, s2;
+};
+struct DiagJob {              // D_seg[a,b] += c * da[a] * db[b]; null pointer = all ones
+    long long seg_off;
+    const double *da, *db;    // first diagonal element
+    long long stride_a, stride_b;    // ld+1
+    int rows, cols;
+    double c;
+};
+
+// ---- Davidson device state (Alg. 3) ----
+constexpr int KMAX = 32;
+struct DavState {
+    double B[KMAX * KMAX];    // row-major, kept symmetric (A18)
+    double y[KMAX];           // lowest eigenvector of B(0:k,0:k)
+    double s[KMAX];           // Gram-Schmidt coefficients / scratch dot products
+    double lambda, rho, rho2, tau2, nx2, x0n2;
+    int done;                 // 1 once ||r|| <= tol
+    int error;                // DMRG_E_NUMERIC sticky
+    int iters;                // applies performed (stops counting once done)
+    int k_used;               // basis size in the last executed step
+    int sweeps;               // Jacobi sweeps of the last small eig
+    int pad[3];
+};
+
+struct Timing { bool enabled = false; cudaEvent_t ev[10]; double ms[8]; bool created = false; };
+
+struct Plan {
+    // problem (host copy)
+    int model = 0; double J = 0, Delta = 0, t = 0, U = 0;
+    int n_labels = 0;
+    std::vector<int> labL, dimL, labR, dimR, target;
+    dmrg_options opt{};
+    // layout
+    long long n = 0;
+    std::vector<int> pairL, pairR;
+    std::vector<long long> segOff;
+    // device memory
+    double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
+    int *counters = nullptr;
+    GemmItem *items1 = nullptr, *items2 = nullptr;
+    GemmUnit *units1 = nullptr, *units2 = nullptr;
+    int n_units1 = 0, n_units2 = 0;
+    // Davidson scratch
+    DavState *state = nullptr;          // device
+    DavState *state_host = nullptr;     // pinned
+    double *tvec = nullptr, *xs = nullptr, *ws = nullptr;   // n doubles each
+    double *partials = nullptr;         // [vec_grid][KMAX+2]
+    int *vec_counter = nullptr;
+    int vec_grid = 0;
+    double *Vown = nullptr, *Wown = nullptr; long long ldv_own = 0;   // dmrg_lowest_eigenpair
+    // stats / misc
+    dmrg_stats stats{};
+    long long device_bytes = 0;
+    std::string err;
+    Timing timing;
+    int sm_count = 148;
+};
+
+void set_global_error(const std::string &s);
+int fail(Plan *p, int code, const std::string &msg);
+
+// plan.cu
+int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out);
+void plan_free(Plan *p);
+
+// gemm.cu
+cudaError_t launch_grouped_gemm(const GemmUnit *units, int n_units, const GemmItem *items,
+                                const BasePtrs &bases, int *counters, const int *done_flag,
+                                cudaStream_t st);
+cudaError_t gemm_kernel_setup();
+
+// davidson.cu
+int dav_init(Plan *p, const double *x0, int argmin_start, double *V, double *W, long long ldv, cudaStream_t st);
+int dav_enqueue_step(Plan *p, double *V, double *W, long long ldv, int k, cudaStream_t st, int *k_next);
+int dav_ritz(Plan *p, const double *V, long long ldv, int k, double *x_out, cudaStream_t st);
+int dav_gemv_trans(Plan *p, const double *V, long long ldv, int k, const double *w, double *out, cudaStream_t st);
+int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s, double *t, double *nrm2, cudaStream_t st);
+int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st);
+
+// probe.cu
+int probe_fp64(int kind, int reps, double *tflops, cudaStream_t st);
+int probe_hbm(long long bytes, int reps, double *gbs, cudaStream_t st);
+
+}  // namespace dmrg

@@ -1,0 +1,534 @@
+// plan.cu -- host planner: admissible sector pairs, operation records grouped by output,
+// operator repacking, work units of the two grouped launches, diag(H_SB), workspaces.
+//
+// PAPER.md:L340-342 (operation records; "A, B are fixed" over the Davidson iteration),
+// L358-363 (Alg. 5 step 1: records and FLOP workload per output; all records of one output
+// stay with one owner -> no merging of outputs), L165-171 (Eq. 11).  The paper's stream
+// interleaving (Alg. 6-7) is replaced by two grouped launches: stage 1 forms the inner
+// product of every two-factor record, stage 2 forms each output tile as ONE product whose
+// K dimension is the concatenation over all records of that output (fixed order, no atomics).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include "internal.h"
+
+namespace dmrg {
+
+static thread_local std::string g_err;
+void set_global_error(const std::string &s) { g_err = s; }
+const std::string &global_error() { return g_err; }
+int fail(Plan *p, int code, const std::string &msg) {
+    if (p) p->err = msg;
+    g_err = msg;
+    return code;
+}
+
+// ---------------------------------------------------------------- plan-time kernels
+__global__ void repack_kernel(RepackJob j, double *pool) {
+    __shared__ double tile[32][33];
+    double *dst = pool + j.dst_off;
+    const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    if (!j.transpose) {
+        for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+            int r = r0 + rr, c = c0 + threadIdx.x;
+            if (r < j.rows && c < j.cols) {
+                double v = j.s1 * j.src1[(long long)r * j.ld1 + c];
+                if (j.src2) v += j.s2 * j.src2[(long long)r * j.ld2 + c];
+                dst[(long long)r * j.ldd + c] = v;
+            }
+        }
+    } else {
+        // dst(r,c) = src(c,r): read src rows c0.., cols r0..
+        for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+            int sr = c0 + rr, sc = r0 + threadIdx.x;   // src row, src col
+            double v = 0.0;
+            if (sr < j.cols && sc < j.rows) {
+                v = j.s1 * j.src1[(long long)sr * j.ld1 + sc];
+                if (j.src2) v += j.s2 * j.src2[(long long)sr * j.ld2 + sc];
+            }
+            tile[rr][threadIdx.x] = v;
+        }
+        __syncthreads();
+        for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+            int r = r0 + rr, c = c0 + threadIdx.x;
+            if (r < j.rows && c < j.cols) dst[(long long)r * j.ldd + c] = tile[threadIdx.x][rr];
+        }
+    }
+}
+
+__global__ void diag_kernel(DiagJob j, double *D) {
+    long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long tot = (long long)j.rows * j.cols;
+    if (idx >= tot) return;
+    int a = (int)(idx / j.cols), b = (int)(idx % j.cols);
+    double va = j.da ? j.da[a * j.stride_a] : 1.0;
+    double vb = j.db ? j.db[b * j.stride_b] : 1.0;
+    D[j.seg_off + idx] += j.c * (va * vb);
+}
+
+// ---------------------------------------------------------------- host helpers
+namespace {
+
+struct PoolEntry { long long off; int rows, cols, ld; };
+struct FactorBlk { int src, dst, entry; };          // entry = pool index
+struct Term { bool A_id, B_id; std::vector<FactorBlk> A, B; };
+struct Record { int A, B, in_pair, out_pair; };      // pool entries or -1 (identity)
+struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; };
+
+inline long long round_up(long long v, long long a) { return (v + a - 1) / a * a; }
+
+struct Builder {
+    Plan *p;
+    const dmrg_problem *pr;
+    std::vector<PoolEntry> pool;
+    std::vector<RepackJob> jobs;
+    long long pool_elems = 0;
+    long long op_elems = 0;
+
+    int add_entry(const dmrg_block_op &op, int b, const std::vector<int> &dims, bool transpose, double scale,
+                  const dmrg_block_op *op2 = nullptr, int b2 = -1, double scale2 = 0.0) {
+        int rs = dims[op.dst[b]], cs = dims[op.src[b]];   // source block shape rs x cs
+        PoolEntry e;
+        e.rows = transpose ? cs : rs;
+        e.cols = transpose ? rs : cs;
+        e.ld = (int)round_up(std::max(e.cols, 1), 2);
+        e.off = pool_elems;
+        pool_elems += round_up((long long)std::max(e.rows, 1) * e.ld, 16);
+        op_elems += (long long)e.rows * e.cols;
+        RepackJob j{};
+        j.src1 = op.data + op.offset[b];
+        j.ld1 = op.ld[b];
+        j.s1 = scale;
+        if (op2) { j.src2 = op2->data + op2->offset[b2]; j.ld2 = op2->ld[b2]; j.s2 = scale2; }
+        j.dst_off = e.off; j.ldd = e.ld; j.rows = e.rows; j.cols = e.cols; j.transpose = transpose ? 1 : 0;
+        jobs.push_back(j);
+        pool.push_back(e);
+        return (int)pool.size() - 1;
+    }
+};
+
+int check_op(Plan *p, const char *name, const dmrg_block_op &op, const std::vector<int> &dims,
+             const std::vector<int> &labs, int nl, bool must_be_diagonal) {
+    int ns = (int)dims.size();
+    if (op.n_blocks < 0) return fail(p, DMRG_E_INVALID_ARG, std::string(name) + ": n_blocks < 0");
+    if (op.n_blocks == 0) return DMRG_OK;
+    if (!op.src || !op.dst || !op.offset || !op.ld || !op.data)
+        return fail(p, DMRG_E_INVALID_ARG, std::string(name) + ": null array with n_blocks > 0");
+    std::vector<int> shift(nl, 0);
+    bool have = false;
+    for (int b = 0; b < op.n_blocks; b++) {
+        int s = op.src[b], d = op.dst[b];
+        if (s < 0 || s >= ns || d < 0 || d >= ns)
+            return fail(p, DMRG_E_SECTOR, std::string(name) + ": block sector index out of range");
+        if (op.ld[b] < dims[s]) return fail(p, DMRG_E_SECTOR, std::string(name) + ": ld smaller than dims[src]");
+        if (op.offset[b] < 0) return fail(p, DMRG_E_INVALID_ARG, std::string(name) + ": negative offset");
+        if (must_be_diagonal && s != d)
+            return fail(p, DMRG_E_SECTOR, std::string(name) + ": must be block-diagonal (src == dst)");
+        for (int a = 0; a < nl; a++) {
+            int sh = labs[d * nl + a] - labs[s * nl + a];
+            if (!have) shift[a] = sh;
+            else if (shift[a] != sh)
+                return fail(p, DMRG_E_SECTOR, std::string(name) + ": blocks with different label shifts (A4)");
+        }
+        have = true;
+    }
+    return DMRG_OK;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------- plan_build
+#define CUDA_TRY(p, x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) { \
+    plan_free(p); return fail(nullptr, (e__ == cudaErrorMemoryAllocation) ? DMRG_E_ALLOC : DMRG_E_CUDA, \
+    std::string(#x) + ": " + cudaGetErrorString(e__)); } } while (0)
+
+template <class T>
+static cudaError_t dev_alloc(Plan *p, T **ptr, long long count) {
+    size_t bytes = (size_t)std::max<long long>(count, 1) * sizeof(T);
+    cudaError_t e = cudaMalloc((void **)ptr, bytes);
+    if (e == cudaSuccess) p->device_bytes += (long long)bytes;
+    return e;
+}
+
+int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
+    *out = nullptr;
+    if (!pr) return fail(nullptr, DMRG_E_INVALID_ARG, "problem is NULL");
+    if (pr->model != DMRG_HEISENBERG && pr->model != DMRG_HUBBARD)
+        return fail(nullptr, DMRG_E_INVALID_ARG, "unknown model");
+    const int nl = pr->left.n_labels;
+    if (nl < 1 || nl > 2 || pr->right.n_labels != nl)
+        return fail(nullptr, DMRG_E_INVALID_ARG, "n_labels must be 1 or 2 and equal on both sides");
+    if (pr->model == DMRG_HUBBARD && nl != 2)
+        return fail(nullptr, DMRG_E_INVALID_ARG, "Hubbard needs two labels (N_up, N_dn)");
+    if (pr->left.n_sectors < 0 || pr->right.n_sectors < 0 || !pr->target)
+        return fail(nullptr, DMRG_E_INVALID_ARG, "bad sector count or NULL target");
+    if ((pr->left.n_sectors && (!pr->left.labels || !pr->left.dims)) ||
+        (pr->right.n_sectors && (!pr->right.labels || !pr->right.dims)))
+        return fail(nullptr, DMRG_E_INVALID_ARG, "NULL sector arrays");
+
+    Plan *p = new Plan();
+    p->model = pr->model; p->J = pr->J; p->Delta = pr->Delta; p->t = pr->t; p->U = pr->U;
+    p->n_labels = nl;
+    if (opts) p->opt = *opts;
+    else { p->opt.k_max = 20; p->opt.tol = 1e-10; p->opt.max_iter = 2000; p->opt.reorth = 1; p->opt.seed = 1; }
+    if (p->opt.k_max == 0) p->opt.k_max = 20;
+    if (p->opt.max_iter <= 0) p->opt.max_iter = 2000;
+    if (p->opt.reorth <= 0) p->opt.reorth = 1;
+    if (p->opt.check_every <= 0) p->opt.check_every = 8;
+    if (p->opt.k_max < 2 || p->opt.k_max > KMAX || p->opt.reorth > 2 || !(p->opt.tol >= 0.0)) {
+        delete p; return fail(nullptr, DMRG_E_INVALID_ARG, "options: need 2 <= k_max <= 32, reorth in {1,2}, tol >= 0");
+    }
+    const int nL = pr->left.n_sectors, nR = pr->right.n_sectors;
+    p->labL.assign(pr->left.labels, pr->left.labels + (size_t)nL * nl);
+    p->labR.assign(pr->right.labels, pr->right.labels + (size_t)nR * nl);
+    p->dimL.assign(pr->left.dims, pr->left.dims + nL);
+    p->dimR.assign(pr->right.dims, pr->right.dims + nR);
+    p->target.assign(pr->target, pr->target + nl);
+    for (int d : p->dimL) if (d < 0) { delete p; return fail(nullptr, DMRG_E_SECTOR, "negative sector dimension"); }
+    for (int d : p->dimR) if (d < 0) { delete p; return fail(nullptr, DMRG_E_SECTOR, "negative sector dimension"); }
+
+    {   // device properties
+        int dev = 0; cudaDeviceProp prop;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+            delete p; return fail(nullptr, DMRG_E_CUDA, "no CUDA device: this library has no CPU fallback");
+        }
+        p->sm_count = prop.multiProcessorCount;
+    }
+
+    // ---- operator validation (A4, A26)
+    struct Chk { const char *nm; const dmrg_block_op *op; bool left; bool diag; };
+    const Chk chks[] = {
+        {"H_L", &pr->H_L, true, true}, {"H_R", &pr->H_R, false, true},
+        {"Sz_L", &pr->Sz_L, true, true}, {"Sp_L", &pr->Sp_L, true, false},
+        {"Sz_R", &pr->Sz_R, false, true}, {"Sp_R", &pr->Sp_R, false, false},
+        {"Cup_L", &pr->Cup_L, true, false}, {"Cdn_L", &pr->Cdn_L, true, false},
+        {"Cup_R", &pr->Cup_R, false, false}, {"Cdn_R", &pr->Cdn_R, false, false},
+        {"D_L", &pr->D_L, true, true}, {"D_R", &pr->D_R, false, true}};
+    for (const Chk &c : chks) {
+        int rc = check_op(nullptr, c.nm, *c.op, c.left ? p->dimL : p->dimR, c.left ? p->labL : p->labR, nl, c.diag);
+        if (rc != DMRG_OK) { delete p; return rc; }
+    }
+
+    // ---- admissible pairs and flat layout (A1, A5)
+    std::map<std::pair<int, int>, int> pair_index;
+    std::vector<std::vector<int>> pairs_of_left(nL);
+    for (int i = 0; i < nL; i++) for (int k = 0; k < nR; k++) {
+        if (p->dimL[i] == 0 || p->dimR[k] == 0) continue;
+        bool ok = true;
+        for (int a = 0; a < nl; a++) ok = ok && (p->labL[i * nl + a] + p->labR[k * nl + a] == p->target[a]);
+        if (!ok) continue;
+        pair_index[{i, k}] = (int)p->pairL.size();
+        pairs_of_left[i].push_back((int)p->pairL.size());
+        p->pairL.push_back(i); p->pairR.push_back(k);
+        p->segOff.push_back(p->n);
+        p->n += (long long)p->dimL[i] * p->dimR[k];
+    }
+    if (p->n == 0) { delete p; return fail(nullptr, DMRG_E_SECTOR, "empty target sector (no admissible pair, A26)"); }
+    const int P = (int)p->pairL.size();
+
+    // ---- terms (reading A3, A6, A7) -> pool entries
+    Builder bl; bl.p = p; bl.pr = pr;
+    std::vector<Term> terms;
+    auto sector_blocks_by_src = [](const dmrg_block_op &op, int ns) {
+        std::vector<std::vector<int>> v(ns);
+        for (int b = 0; b < op.n_blocks; b++) v[op.src[b]].push_back(b);
+        return v;
+    };
+    {   // H_L (+ U D_L) (x) I   and   I (x) H_R (+ U D_R)
+        for (int side = 0; side < 2; side++) {
+            const dmrg_block_op &H = side == 0 ? pr->H_L : pr->H_R;
+            const dmrg_block_op &Dd = side == 0 ? pr->D_L : pr->D_R;
+            const std::vector<int> &dims = side == 0 ? p->dimL : p->dimR;
+            const bool useD = (pr->model == DMRG_HUBBARD) && Dd.n_blocks > 0 && pr->U != 0.0;
+            Term t; t.A_id = side == 1; t.B_id = side == 0;
+            auto hs = sector_blocks_by_src(H, (int)dims.size());
+            auto ds = sector_blocks_by_src(Dd, (int)dims.size());
+            for (int s = 0; s < (int)dims.size(); s++) {
+                if (dims[s] == 0) continue;
+                // several blocks on one sector are summed pairwise at most (one H, one D)
+                if (hs[s].size() > 1 || ds[s].size() > 1) {
+                    delete p; return fail(nullptr, DMRG_E_SECTOR, "H/D: more than one block on a sector");
+                }
+                int e = -1;
+                const bool tr = side == 1;   // right factors are stored as B^T
+                if (!hs[s].empty() && useD && !ds[s].empty())
+                    e = bl.add_entry(H, hs[s][0], dims, tr, 1.0, &Dd, ds[s][0], pr->U);
+                else if (!hs[s].empty())
+                    e = bl.add_entry(H, hs[s][0], dims, tr, 1.0);
+                else if (useD && !ds[s].empty())
+                    e = bl.add_entry(Dd, ds[s][0], dims, tr, pr->U);
+                if (e >= 0) (side == 0 ? t.A : t.B).push_back({s, s, e});
+            }
+            terms.push_back(std::move(t));
+        }
+    }
+    auto parity_sign = [&](int left_sector) {
+        int N = 0;
+        for (int a = 0; a < nl; a++) N += p->labL[left_sector * nl + a];
+        return (N % 2 == 0) ? 1.0 : -1.0;
+    };
+    if (pr->model == DMRG_HEISENBERG) {
+        const double half = 0.5 * pr->J, zz = pr->J * pr->Delta;
+        if (pr->Sp_L.n_blocks && pr->Sp_R.n_blocks && half != 0.0) {
+            Term tp; tp.A_id = tp.B_id = false;   // S+_L (x) S-_R
+            Term tm; tm.A_id = tm.B_id = false;   // S-_L (x) S+_R
+            for (int b = 0; b < pr->Sp_L.n_blocks; b++) {
+                int s = pr->Sp_L.src[b], d = pr->Sp_L.dst[b];
+                if (!p->dimL[s] || !p->dimL[d]) continue;
+                tp.A.push_back({s, d, bl.add_entry(pr->Sp_L, b, p->dimL, false, half)});
+                tm.A.push_back({d, s, bl.add_entry(pr->Sp_L, b, p->dimL, true, half)});
+            }
+            for (int b = 0; b < pr->Sp_R.n_blocks; b++) {
+                int s = pr->Sp_R.src[b], d = pr->Sp_R.dst[b];
+                if (!p->dimR[s] || !p->dimR[d]) continue;
+                // S-_R block d->s has matrix blk^T, so its B^T is blk as stored
+                tp.B.push_back({d, s, bl.add_entry(pr->Sp_R, b, p->dimR, false, 1.0)});
+                tm.B.push_back({s, d, bl.add_entry(pr->Sp_R, b, p->dimR, true, 1.0)});
+            }
+            terms.push_back(std::move(tp));
+            terms.push_back(std::move(tm));
+        }
+        if (pr->Sz_L.n_blocks && pr->Sz_R.n_blocks && zz != 0.0) {
+            Term tz; tz.A_id = tz.B_id = false;
+            for (int b = 0; b < pr->Sz_L.n_blocks; b++)
+                if (p->dimL[pr->Sz_L.src[b]])
+                    tz.A.push_back({pr->Sz_L.src[b], pr->Sz_L.dst[b], bl.add_entry(pr->Sz_L, b, p->dimL, false, zz)});
+            for (int b = 0; b < pr->Sz_R.n_blocks; b++)
+                if (p->dimR[pr->Sz_R.src[b]])
+                    tz.B.push_back({pr->Sz_R.src[b], pr->Sz_R.dst[b], bl.add_entry(pr->Sz_R, b, p->dimR, true, 1.0)});
+            terms.push_back(std::move(tz));
+        }
+    } else {
+        const dmrg_block_op *CL[2] = {&pr->Cup_L, &pr->Cdn_L};
+        const dmrg_block_op *CR[2] = {&pr->Cup_R, &pr->Cdn_R};
+        for (int sg = 0; sg < 2; sg++) {
+            if (!CL[sg]->n_blocks || !CR[sg]->n_blocks || pr->t == 0.0) continue;
+            Term t1; t1.A_id = t1.B_id = false;   // -t (c+_L P_L) (x) c_R : sign from the INPUT left sector
+            Term t2; t2.A_id = t2.B_id = false;   // -t (P_L c_L) (x) c+_R : sign from the OUTPUT left sector
+            for (int b = 0; b < CL[sg]->n_blocks; b++) {
+                int s = CL[sg]->src[b], d = CL[sg]->dst[b];
+                if (!p->dimL[s] || !p->dimL[d]) continue;
+                const double c = -pr->t * parity_sign(s);   // s = input of c+, = output of c
+                t1.A.push_back({s, d, bl.add_entry(*CL[sg], b, p->dimL, false, c)});
+                t2.A.push_back({d, s, bl.add_entry(*CL[sg], b, p->dimL, true, c)});
+            }
+            for (int b = 0; b < CR[sg]->n_blocks; b++) {
+                int s = CR[sg]->src[b], d = CR[sg]->dst[b];
+                if (!p->dimR[s] || !p->dimR[d]) continue;
+                t1.B.push_back({d, s, bl.add_entry(*CR[sg], b, p->dimR, false, 1.0)});   // c_R: B^T = blk
+                t2.B.push_back({s, d, bl.add_entry(*CR[sg], b, p->dimR, true, 1.0)});    // c+_R: B^T = blk^T
+            }
+            terms.push_back(std::move(t1));
+            terms.push_back(std::move(t2));
+        }
+    }
+
+    // ---- operation records, in term order, grouped later by output
+    std::vector<Record> recs;
+    for (const Term &t : terms) {
+        if (t.B_id) {
+            for (const FactorBlk &a : t.A)
+                for (int ip : pairs_of_left[a.src]) {
+                    auto it = pair_index.find({a.dst, p->pairR[ip]});
+                    if (it != pair_index.end()) recs.push_back({a.entry, -1, ip, it->second});
+                }
+        } else if (t.A_id) {
+            for (int ip = 0; ip < P; ip++)
+                for (const FactorBlk &b : t.B) {
+                    if (b.src != p->pairR[ip]) continue;
+                    auto it = pair_index.find({p->pairL[ip], b.dst});
+                    if (it != pair_index.end()) recs.push_back({-1, b.entry, ip, it->second});
+                }
+        } else {
+            for (const FactorBlk &a : t.A)
+                for (int ip : pairs_of_left[a.src])
+                    for (const FactorBlk &b : t.B) {
+                        if (b.src != p->pairR[ip]) continue;
+                        auto it = pair_index.find({a.dst, b.dst});
+                        if (it != pair_index.end()) recs.push_back({a.entry, b.entry, ip, it->second});
+                    }
+        }
+    }
+
+    // ---- stage-1 tasks / stage-2 items; association order by FLOP (A24)
+    std::vector<GemmItem> items1, items2;
+    std::vector<TaskHost> tasks1, tasks2;
+    std::vector<std::vector<GemmItem>> out_items(P);
+    long long tws_elems = 0, flops = 0;
+    int n_gemms = 0;
+    auto vec2 = [](long long off, int ld) { return (uint8_t)((off % 2 == 0 && ld % 2 == 0) ? 1 : 0); };
+    for (const Record &r : recs) {
+        const int i = p->pairL[r.in_pair], k = p->pairR[r.in_pair];
+        const int j = p->pairL[r.out_pair], l = p->pairR[r.out_pair];
+        const long long di = p->dimL[i], dk = p->dimR[k], dj = p->dimL[j], dl = p->dimR[l];
+        const long long xoff = p->segOff[r.in_pair];
+        GemmItem it2{};
+        if (r.B < 0) {            // A (x) I :  X'_jk += A X_ik
+            const PoolEntry &A = bl.pool[r.A];
+            it2 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
+            flops += 2 * dj * di * dk; n_gemms += 1;
+        } else if (r.A < 0) {     // I (x) B :  X'_il += X_ik B^T
+            const PoolEntry &B = bl.pool[r.B];
+            it2 = {xoff, B.off, (int)dk, B.ld, (int)dk, BASE_X, BASE_POOL, vec2(xoff, (int)dk), vec2(B.off, B.ld)};
+            flops += 2 * di * dk * dl; n_gemms += 1;
+        } else {
+            const PoolEntry &A = bl.pool[r.A], &B = bl.pool[r.B];
+            const long long f1 = 2 * di * dk * dl + 2 * dj * di * dl;   // T = X B^T ; X' += A T
+            const long long f2 = 2 * dj * di * dk + 2 * dj * dk * dl;   // T = A X   ; X' += T B^T
+            n_gemms += 2;
+            GemmItem it1{};
+            TaskHost t1{};
+            if (f1 <= f2) {
+                const int ldt = (int)round_up(dl, 2);
+                const long long toff = tws_elems; tws_elems += round_up(di * ldt, 16);
+                it1 = {xoff, B.off, (int)dk, B.ld, (int)dk, BASE_X, BASE_POOL, vec2(xoff, (int)dk), vec2(B.off, B.ld)};
+                t1 = {BASE_T, toff, ldt, (int)di, (int)dl, 0, 1};
+                it2 = {A.off, toff, A.ld, ldt, (int)di, BASE_POOL, BASE_T, vec2(A.off, A.ld), 1};
+                flops += f1;
+            } else {
+                const int ldt = (int)round_up(dk, 2);
+                const long long toff = tws_elems; tws_elems += round_up(dj * ldt, 16);
+                it1 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
+                t1 = {BASE_T, toff, ldt, (int)dj, (int)dk, 0, 1};
+                it2 = {toff, B.off, ldt, B.ld, (int)dk, BASE_T, BASE_POOL, 1, vec2(B.off, B.ld)};
+                flops += f2;
+            }
+            t1.item_begin = (int)items1.size();
+            items1.push_back(it1);
+            tasks1.push_back(t1);
+        }
+        out_items[r.out_pair].push_back(it2);
+    }
+    for (int op = 0; op < P; op++) {
+        TaskHost t{};
+        t.c_base = BASE_Y; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
+        t.M = p->dimL[p->pairL[op]]; t.N = p->dimR[p->pairR[op]];
+        t.item_begin = (int)items2.size(); t.item_count = (int)out_items[op].size();
+        for (const GemmItem &it : out_items[op]) items2.push_back(it);
+        tasks2.push_back(t);   // outputs without any record are still zero-filled by the kernel
+    }
+
+    // ---- work units: tiles x split of the concatenated K (fixed-order second-stage reduce)
+    long long part_elems = 0; int n_counters = 0; int split_tiles2 = 0;
+    auto make_units = [&](const std::vector<TaskHost> &tasks, const std::vector<GemmItem> &items,
+                          std::vector<GemmUnit> &units, int *split_tiles) {
+        long long W = 0;
+        for (const TaskHost &t : tasks) {
+            int kt = 0;
+            for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
+            W += (long long)kt * ((t.M + BM - 1) / BM) * ((t.N + BN - 1) / BN);
+        }
+        const int kt_min = 8;
+        long long kt_unit = std::max<long long>(kt_min, (W + (long long)p->sm_count * 8 - 1) / ((long long)p->sm_count * 8));
+        for (const TaskHost &t : tasks) {
+            int kt = 0;
+            for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
+            for (int m0 = 0; m0 < t.M; m0 += BM) for (int n0 = 0; n0 < t.N; n0 += BN) {
+                int ns = (int)std::max<long long>(1, (kt + kt_unit - 1) / kt_unit);
+                // never split below kt_min k-tiles per unit
+                while (ns > 1 && kt / ns < kt_min) ns--;
+                int tile_id = -1; long long poff = 0;
+                if (ns > 1) { tile_id = n_counters++; poff = part_elems; part_elems += (long long)ns * BM * BN; if (split_tiles) (*split_tiles)++; }
+                int base = kt / ns, rem = kt % ns, begin = 0;
+                for (int s = 0; s < ns; s++) {
+                    GemmUnit u{};
+                    u.c_off = t.c_off; u.part_off = poff; u.ldc = t.ldc; u.M = t.M; u.N = t.N; u.m0 = m0; u.n0 = n0;
+                    u.item_begin = t.item_begin; u.item_count = t.item_count;
+                    u.kt_begin = begin; u.kt_count = base + (s < rem ? 1 : 0); begin += u.kt_count;
+                    u.tile_id = tile_id; u.split_idx = s; u.n_split = ns;
+                    u.c_base = t.c_base; u.c_vec2 = vec2(t.c_off, t.ldc);
+                    units.push_back(u);
+                }
+            }
+        }
+        std::stable_sort(units.begin(), units.end(), [](const GemmUnit &a, const GemmUnit &b) { return a.kt_count > b.kt_count; });
+    };
+    std::vector<GemmUnit> units1, units2;
+    make_units(tasks1, items1, units1, nullptr);
+    make_units(tasks2, items2, units2, &split_tiles2);
+
+    // ---- device allocations
+    CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
+    CUDA_TRY(p, dev_alloc(p, &p->tws, tws_elems));
+    CUDA_TRY(p, dev_alloc(p, &p->part, part_elems));
+    CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
+    CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->items1, (long long)items1.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->items2, (long long)items2.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->units1, (long long)units1.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->units2, (long long)units2.size()));
+    CUDA_TRY(p, cudaMemset(p->pool, 0, sizeof(double) * std::max<long long>(bl.pool_elems, 1)));
+    CUDA_TRY(p, cudaMemset(p->tws, 0, sizeof(double) * std::max<long long>(tws_elems, 1)));
+    CUDA_TRY(p, cudaMemset(p->counters, 0, sizeof(int) * std::max(n_counters, 1)));
+    CUDA_TRY(p, cudaMemset(p->D, 0, sizeof(double) * p->n));
+    if (!items1.empty()) CUDA_TRY(p, cudaMemcpy(p->items1, items1.data(), items1.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
+    if (!items2.empty()) CUDA_TRY(p, cudaMemcpy(p->items2, items2.data(), items2.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
+    if (!units1.empty()) CUDA_TRY(p, cudaMemcpy(p->units1, units1.data(), units1.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
+    if (!units2.empty()) CUDA_TRY(p, cudaMemcpy(p->units2, units2.data(), units2.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
+    p->n_units1 = (int)units1.size(); p->n_units2 = (int)units2.size();
+
+    // ---- repack the operators (scaled / transposed / aligned), once
+    for (const RepackJob &j : bl.jobs) {
+        if (j.rows == 0 || j.cols == 0) continue;
+        dim3 grid((j.cols + 31) / 32, (j.rows + 31) / 32), block(32, 8);
+        repack_kernel<<<grid, block>>>(j, p->pool);
+    }
+    CUDA_TRY(p, cudaGetLastError());
+
+    // ---- diag(H_SB) (A14): records with (i,k) == (j,l)
+    for (const Record &r : recs) {
+        if (r.in_pair != r.out_pair) continue;
+        DiagJob dj{};
+        dj.seg_off = p->segOff[r.in_pair];
+        dj.rows = p->dimL[p->pairL[r.in_pair]]; dj.cols = p->dimR[p->pairR[r.in_pair]];
+        dj.c = 1.0;   // the coefficient is already folded into the left factor
+        if (r.A >= 0) { dj.da = p->pool + bl.pool[r.A].off; dj.stride_a = bl.pool[r.A].ld + 1; }
+        if (r.B >= 0) { dj.db = p->pool + bl.pool[r.B].off; dj.stride_b = bl.pool[r.B].ld + 1; }
+        long long tot = (long long)dj.rows * dj.cols;
+        diag_kernel<<<(unsigned)((tot + 255) / 256), 256>>>(dj, p->D);
+    }
+    CUDA_TRY(p, cudaGetLastError());
+
+    // ---- Davidson scratch
+    p->vec_grid = (int)std::max<long long>(1, std::min<long long>((long long)p->sm_count * 4, (p->n + 511) / 512));
+    CUDA_TRY(p, dev_alloc(p, &p->state, 1));
+    CUDA_TRY(p, cudaMemset(p->state, 0, sizeof(DavState)));
+    CUDA_TRY(p, cudaMallocHost((void **)&p->state_host, sizeof(DavState)));
+    memset(p->state_host, 0, sizeof(DavState));
+    CUDA_TRY(p, dev_alloc(p, &p->tvec, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->xs, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->ws, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->partials, (long long)p->vec_grid * (KMAX + 2)));
+    CUDA_TRY(p, dev_alloc(p, &p->vec_counter, 4));
+    CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
+    CUDA_TRY(p, gemm_kernel_setup());
+    CUDA_TRY(p, cudaDeviceSynchronize());
+
+    // ---- stats
+    dmrg_stats &s = p->stats;
+    s.n = p->n; s.n_pairs = P; s.n_records = (int)recs.size(); s.n_gemms = n_gemms;
+    s.flop_per_apply = flops; s.operator_elems = bl.op_elems; s.apply_bytes = 8 * (bl.op_elems + 2 * p->n);
+    s.stage1_units = p->n_units1; s.stage2_units = p->n_units2; s.stage2_split_tiles = split_tiles2;
+    s.pool_bytes = 8 * bl.pool_elems;
+    s.workspace_bytes = 8 * (tws_elems + part_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
+    s.device_bytes = p->device_bytes;
+    s.kernel_launches_per_apply = (p->n_units1 > 0 ? 1 : 0) + 1;
+    s.kernel_launches_per_step = s.kernel_launches_per_apply + 5 + 2 * p->opt.reorth;
+    *out = p;
+    return DMRG_OK;
+}
+
+void plan_free(Plan *p) {
+    if (!p) return;
+    cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
+    cudaFree(p->items1); cudaFree(p->items2); cudaFree(p->units1); cudaFree(p->units2);
+    cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
+    cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
+    cudaFree(p->Vown); cudaFree(p->Wown);
+    if (p->timing.created) for (auto &e : p->timing.ev) cudaEventDestroy(e);
+    delete p;
+}
+
+}  // namespace dmrg
