@@ -1,0 +1,231 @@
+"""Parity of the Davidson side (Alg. 3) with the CPU oracle O-DAV.
+
+Protocol (reading A20): (i) the BLAS-2 kernels against numpy; (ii) lock-step: the GPU's own
+(V, W, B, k) is handed to one oracle step and lambda, ||r||, the new column of B and the appended vector are
+compared; (iii) from the deterministic start e_argmin(D) whole trajectories are compared iteration by
+iteration; (iv) converged eigenpairs: |d lambda| <= 1e-9, |<x_gpu, x_oracle>| >= 1 - 1e-6 (north_star)."""
+import numpy as np
+import pytest
+
+from dmrg_inputs import random_vector
+from dmrg_inputs.synthetic import vector_seed
+from oracle import blocks, rec, kron, davidson as odav
+from gpu_common import (small_problems, full_config, oracle_apply, to_dev, basis_to_numpy,
+                        LAMBDA_ATOL, OVERLAP_DEF)
+
+pytestmark = pytest.mark.gpu
+SMALL = small_problems()
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1309_5571_b200 as lib
+    lib.load_library()
+    return lib
+
+
+@pytest.mark.parametrize("ldv_pad", [0, 1, 16])
+def test_blas2_kernels_match_numpy(lib, ldv_pad):
+    """gemv_trans (Alg. 3 lines 3, 12) and gemv (line 13) for every basis size 1..32, ragged n, odd ldv."""
+    import torch
+    p = SMALL["cfg2_m160"]()
+    plan = lib.Plan(p, k_max=32)
+    n = plan.n
+    rng = np.random.default_rng(4)
+    ldv = n + ldv_pad
+    Vh = rng.standard_normal((32, ldv)); wh = rng.standard_normal(n); sh = rng.standard_normal(32)
+    V = to_dev(Vh); w = to_dev(wh)
+    for k in range(1, 33):
+        out = plan.gemv_trans(V, k, w).cpu().numpy()
+        ref = Vh[:k, :n] @ wh
+        assert np.max(np.abs(out - ref)) <= 1e-12 * np.sqrt(n) * 4
+        t = to_dev(wh.copy())
+        nrm2 = plan.gemv_sub(V, k, to_dev(sh), t).cpu().numpy()[0]
+        tref = wh - Vh[:k, :n].T @ sh[:k]
+        assert np.max(np.abs(t.cpu().numpy() - tref)) <= 1e-12 * 32
+        assert abs(nrm2 - tref @ tref) <= 1e-12 * (tref @ tref)
+    # bitwise reproducible
+    a = plan.gemv_trans(V, 17, w).clone(); b = plan.gemv_trans(V, 17, w).clone()
+    assert torch.equal(a, b)
+    plan.close()
+
+
+def _lockstep(lib, p, k_max, steps, x0, reorth=1, tol=1e-10):
+    """Runs `steps` GPU steps; before each, snapshots the GPU state and runs ONE oracle step from it."""
+    import torch
+    lay = rec.Layout(p)
+    apply_o = oracle_apply(p, lay)
+    D = rec.diag_H(p, lay)
+    plan = lib.Plan(p, k_max=k_max, tol=tol, reorth=reorth)
+    V, W = plan.new_basis()
+    plan.davidson_init(V, W, x0=None if x0 is None else to_dev(x0), start_at_argmin_diag=x0 is None)
+    k = 1
+    n = plan.n
+    worst = dict(lam=0.0, rho=0.0, B=0.0, v=0.0)
+    for it in range(steps):
+        B0, _ = plan.get_small()
+        st = odav.DavidsonState(basis_to_numpy(V, n, k_max).copy(order="F"), basis_to_numpy(W, n, k_max).copy(order="F"),
+                                B0.copy(), k)
+        ores = odav.davidson_step(st, apply_o, D, tol, reorth)
+        k_new, lam, rho, conv = plan.davidson_step(V, W, k)
+        assert conv == ores["converged"]
+        worst["lam"] = max(worst["lam"], abs(lam - ores["lam"]))
+        worst["rho"] = max(worst["rho"], abs(rho - ores["resnorm"]) / (1e-9 + 1e-6 * ores["resnorm"]))
+        B1, y = plan.get_small()
+        if not conv:
+            assert k_new == st.k
+            if k < k_max:   # the new column of B (after a restart B is [lambda])
+                worst["B"] = max(worst["B"], np.max(np.abs(B1[:k, k - 1] - st.B[:k, k - 1])))
+            else:
+                assert abs(B1[0, 0] - ores["lam"]) <= LAMBDA_ATOL and np.count_nonzero(B1) == 1
+            # appended vector, sign-aligned (A18: the sign of y is a convention, ties may flip it)
+            vg = V[k_new - 1, :n].cpu().numpy(); vo = st.V[:, k_new - 1]
+            sgn = 1.0 if vg @ vo >= 0 else -1.0
+            gap = np.min(np.abs(ores["lam"] - D))
+            if gap > 1e-3:   # A20: else the preconditioned vector is legitimately ill-conditioned
+                worst["v"] = max(worst["v"], np.max(np.abs(sgn * vg - vo)))
+        k = k_new
+        if conv:
+            break
+    plan.close()
+    return worst
+
+
+@pytest.mark.parametrize("name,k_max,reorth", [("cfg1", 16, 1), ("cfg1", 5, 2), ("cfg2_m160", 8, 1), ("cfg4_m243", 6, 1),
+                                               ("hub_exact_3_3", 7, 1)])
+def test_lockstep_random_start(lib, name, k_max, reorth):
+    p = SMALL[name]()
+    n = rec.Layout(p).n
+    worst = _lockstep(lib, p, k_max, 25, random_vector(n, 2001), reorth)
+    assert worst["lam"] <= LAMBDA_ATOL and worst["rho"] <= 1.0 and worst["B"] <= 1e-10 and worst["v"] <= 1e-7, worst
+
+
+def test_lockstep_argmin_start(lib):
+    worst = _lockstep(lib, SMALL["hub_syn_m400"](), 9, 30, None)
+    assert worst["lam"] <= LAMBDA_ATOL and worst["rho"] <= 1.0 and worst["B"] <= 1e-10 and worst["v"] <= 1e-7, worst
+
+
+def _trajectory(lib, p, k_max, iters, tol=1e-10):
+    """GPU and oracle run independently from start (D); returns both (lambda, ||r||) histories."""
+    lay = rec.Layout(p)
+    D = rec.diag_H(p, lay)
+    ores = odav.davidson_solve(oracle_apply(p, lay), D, odav.start_argmin_diag(D), k_max, tol, iters)
+    plan = lib.Plan(p, k_max=k_max, tol=tol)
+    V, W = plan.new_basis()
+    plan.davidson_init(V, W, start_at_argmin_diag=True)
+    # the start is e_argmin(D) exactly
+    v0 = V[0, :plan.n].cpu().numpy()
+    assert v0[int(np.argmin(D))] == 1.0 and np.count_nonzero(v0) == 1
+    k, hist = 1, []
+    for it in range(iters):
+        k, lam, rho, conv = plan.davidson_step(V, W, k)
+        hist.append((lam, rho))
+        if conv:
+            break
+    x = plan.ritz_vector(V, k).cpu().numpy() if hist and conv else None
+    plan.close()
+    return hist, ores, x
+
+
+@pytest.mark.parametrize("name,k_max,iters", [("cfg1", 16, 200), ("cfg2_m160", 16, 60), ("cfg4_m243", 16, 60)])
+def test_trajectory_parity_small(lib, name, k_max, iters):
+    hist, ores, x = _trajectory(lib, SMALL[name](), k_max, iters)
+    oh = ores["history"]
+    assert abs(len(hist) - len(oh)) <= 1
+    for (lg, rg), (lo, ro) in zip(hist, oh):
+        assert abs(lg - lo) <= LAMBDA_ATOL
+        assert abs(rg - ro) <= 1e-9 + 1e-6 * ro
+    if ores["converged"] and x is not None:
+        assert abs(abs(x @ ores["x"]) - 1.0) <= OVERLAP_DEF
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg3"])
+def test_trajectory_parity_full_config(lib, name):
+    """BASELINE.json configs at full size, deterministic start, fixed iteration count (A20)."""
+    from dmrg_inputs import CONFIGS
+    iters = {"cfg2": 50, "cfg4": 50, "cfg3": 40}[name]
+    hist, ores, _ = _trajectory(lib, full_config(name), CONFIGS[name]["k_max"], iters)
+    assert len(hist) == len(ores["history"]) == iters
+    for (lg, rg), (lo, ro) in zip(hist, ores["history"]):
+        assert abs(lg - lo) <= LAMBDA_ATOL
+        assert abs(rg - ro) <= 1e-9 + 1e-6 * ro
+
+
+def test_cfg1_eigenpair_vs_exact_diagonalisation(lib):
+    """Config 1: lowest eigenpair from the seeded random start equals the full 4096x4096 ED ground state."""
+    p = SMALL["cfg1"]()
+    Hs, _ = kron.H_sector(p)
+    w, v = np.linalg.eigh(Hs)
+    plan = lib.Plan(p, k_max=16, tol=1e-10)
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(to_dev(random_vector(plan.n, vector_seed("cfg2", "start") - 1)))
+    assert rc == lib.DMRG_OK and rho <= 1e-10 and 10 < iters < 200
+    assert abs(lam - w[0]) <= LAMBDA_ATOL and abs(lam - (-5.142090632841)) <= LAMBDA_ATOL
+    xg = x.cpu().numpy()
+    assert abs(np.linalg.norm(xg) - 1) <= 1e-12
+    assert abs(xg @ v[:, 0]) >= 1 - OVERLAP_DEF
+    # device-generated seeded start and the argmin start reach the same state
+    for kw in (dict(), dict(start_at_argmin_diag=True)):
+        rc2, lam2, x2, _, _ = plan.lowest_eigenpair(None, **kw)
+        assert rc2 == lib.DMRG_OK and abs(lam2 - w[0]) <= LAMBDA_ATOL and abs(x2.cpu().numpy() @ v[:, 0]) >= 1 - OVERLAP_DEF
+    # driver == step-by-step: same iteration count and eigenvalue bits from the same start
+    x0 = to_dev(random_vector(plan.n, 11))
+    rc3, lam3, _, _, it3 = plan.lowest_eigenpair(x0)
+    V, W = plan.new_basis(); plan.davidson_init(V, W, x0=x0)
+    k = 1
+    for it in range(1, 400):
+        k, lam, rho, conv = plan.davidson_step(V, W, k)
+        if conv:
+            break
+    assert it == it3 and lam == lam3
+    plan.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_converged_eigenpair_full_config(lib, name):
+    """Converged lowest eigenpair at full size, random start (R), vs the oracle's own Davidson run."""
+    from dmrg_inputs import CONFIGS
+    p = full_config(name)
+    lay = rec.Layout(p)
+    D = rec.diag_H(p, lay)
+    x0 = random_vector(lay.n, vector_seed(name, "start"))
+    k_max = CONFIGS[name]["k_max"]
+    ores = odav.davidson_solve(oracle_apply(p, lay), D, x0, k_max, 1e-10, 3000)
+    assert ores["converged"]
+    plan = lib.Plan(p, k_max=k_max, tol=1e-10, max_iter=3000)
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(to_dev(x0))
+    assert rc == lib.DMRG_OK and rho <= 1e-10
+    assert abs(lam - ores["lam"]) <= LAMBDA_ATOL
+    assert abs(x.cpu().numpy() @ ores["x"]) >= 1 - OVERLAP_DEF
+    plan.close()
+
+
+def test_cfg3_converged_eigenpair_properties(lib):
+    """Config 3: the oracle checks the converged GPU eigenpair (Rayleigh quotient, residual) with its own apply."""
+    p = full_config("cfg3")
+    lay = rec.Layout(p)
+    plan = lib.Plan(p, k_max=24, tol=1e-10, max_iter=3000)
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(None, start_at_argmin_diag=True)
+    assert rc == lib.DMRG_OK
+    xg = x.cpu().numpy()
+    Hx = oracle_apply(p, lay)(xg)
+    assert abs(xg @ Hx - lam) <= LAMBDA_ATOL
+    assert np.linalg.norm(Hx - lam * xg) <= 1e-9
+    plan.close()
+
+
+def test_not_converged_and_breakdown_codes(lib):
+    import torch
+    p = SMALL["cfg2_m160"]()
+    plan = lib.Plan(p, k_max=4, tol=1e-14, max_iter=5, check_every=2)
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(None, start_at_argmin_diag=True)
+    assert rc == lib.DMRG_NOT_CONVERGED and iters == 5 and rho > 1e-14
+    assert abs(float(x.norm()) - 1.0) <= 1e-12
+    # zero start vector -> NUMERIC (zero norm)
+    V, W = plan.new_basis()
+    plan.davidson_init(V, W, x0=torch.zeros(plan.n, dtype=torch.float64, device="cuda"))
+    with pytest.raises(lib.DmrgError) as e:
+        plan.davidson_step(V, W, 1)
+    assert e.value.code == lib.DMRG_E_NUMERIC
+    plan.close()
