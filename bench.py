@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the DMRG hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config cfg3]
+
+Workload (BASELINE.json configs[2], the one the metric is quoted on: "m=2048"): Heisenberg
+spin-1/2, Delta=0.5, synthetic blocks m=2048 per side, Sz sectors -16..16, target Sz=0
+(n ~ 7.3e5), Davidson basis limit k_max=24, deterministic start e_argmin(D).  Inputs are seeded
+and synthetic.
+
+A step = one call of Alg. 3 = one pass of the whole hot path: the projection
+W(:,k) = H_SB V(:,k) (two grouped DMMA launches) plus every BLAS-2 row of SURVEY 8(a) (V^T w, small
+eig, residual + preconditioner, Gram-Schmidt, normalise/append, restart collapse when due), through
+the C ABI (dmrg_davidson_step), basis size cycling 1..k_max as in a real run.
+
+value   = algorithmic FP64 GFLOP/s of the whole step (A24 FLOP of the apply + BLAS-2 FLOP) with
+          everything resident in HBM; L2 is flushed between timed steps (outside the event pairs).
+e2e     = same metric with host buffers: every step copies the newest basis vector host->device from
+          pinned memory and the projected vector W(:,k) device->host (the per-iteration crossing of the
+          paper's hybrid scheme: H2D of the input, D2H of the output, Alg. 7).
+roofline= the grouped DMMA kernel (both launches of a step) against the FP64 DMMA peak measured live.
+cpu_baseline / --impl reference = the oracle's O-DAV iteration (oracle/, numpy) on the host cores.
+"""
+from __future__ import annotations
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "fp64_gflops_davidson_iteration"   # H*psi + Davidson BLAS-2, algorithmic FLOP / time
+UNIT = "GFLOP/s"
+
+
+def blas2_flop(n: int, k: int, k_eff: int, reorth: int) -> float:
+    """FLOP of the BLAS-2 rows of one step: V^T w 2nk; x, Wy 4nk (+4n); reorth x (2nk' + 2nk' + 2n); n."""
+    return 2.0 * n * k + 4.0 * n * k + 4.0 * n + reorth * (4.0 * n * k_eff + 2.0 * n) + n
+
+
+def blas2_bytes(n: int, k: int, k_eff: int, reorth: int, restart: bool) -> float:
+    """Algorithmic bytes of the BLAS-2 rows of one step."""
+    b = 8.0 * n * (k + 1)                       # a3  V^T w
+    b += 8.0 * n * (2 * k) + 16.0 * n           # a5-a7 fused: V, W, D read, t written
+    if restart:
+        b += 16.0 * n + 32.0 * n                # x, Wy written; collapse reads them and writes V0, W0
+    b += reorth * (8.0 * n * (k_eff + 1) + 8.0 * n * (k_eff + 1) + 8.0 * n)   # a8
+    b += 16.0 * n                               # a9
+    return b
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [t.strip() for t in line.split(",")]))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = [float(r[0]) for r in rows]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for j, nm in enumerate(names) if any(r[3 + j].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "samples": len(rows), "power_w_max": max(float(r[2]) for r in rows)}
+
+
+def make_problem(name: str):
+    from dmrg_inputs import make_config, CONFIGS
+    return make_config(name), CONFIGS[name]
+
+
+def oracle_iteration_timer(problem, k_max: int, steps: int, warmup: int):
+    """Times the oracle's O-DAV step (oracle/davidson.py on oracle/rec.py) as it stands."""
+    from oracle import rec, davidson as odav
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([d.get("num_threads", 1) for d in threadpool_info()] or [os.cpu_count() or 1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    lay = rec.Layout(problem)
+    recs = rec.records(problem, lay)
+    D = rec.diag_H(problem, lay)
+    apply_o = lambda v: rec.apply_blockwise(problem, v, lay, recs)
+    st = odav.init_state(odav.start_argmin_diag(D), k_max)
+    flop_apply = rec.flop_count(problem, lay)
+    times, flops = [], []
+    for it in range(warmup + steps):
+        k = st.k
+        k_eff = 1 if k == k_max else k
+        t0 = time.perf_counter()
+        res = odav.davidson_step(st, apply_o, D, 1e-10, 1)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+            flops.append(flop_apply + blas2_flop(lay.n, k, k_eff, 1))
+        if res["converged"]:
+            st = odav.init_state(odav.start_argmin_diag(D), k_max)
+    return sum(flops) / sum(times) / 1e9, sum(times) / len(times) * 1e3, cores, lay.n
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    problem, cfg = make_problem(args.config)
+    steps = min(args.steps, 60)
+    gfl, ms, cores, n = oracle_iteration_timer(problem, cfg["k_max"], steps, max(1, min(args.warmup, 3)))
+    line = {"impl": "reference", "metric": METRIC, "value": gfl, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args.config, cfg, n, None),
+            "cpu_baseline": {"value": gfl, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{steps} consecutive O-DAV iterations (oracle/davidson.py on oracle/rec.py) of {args.config} from start e_argmin(D)"},
+            "e2e": {"value": gfl, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(name, cfg, n, stats):
+    c = {"workload": f"{name}: {cfg['kind']} m={cfg['m']} per side, k_max={cfg['k_max']}, target sector dim n={n}, "
+                     "one Davidson iteration (Alg. 3) per step, start e_argmin(D)",
+         "l2": "flushed between timed steps (256 MiB memset outside the event pairs)", "parallelism": "replicas only"}
+    if stats:
+        c.update({"n_records": stats["n_records"], "n_gemms": stats["n_gemms"], "flop_per_apply": stats["flop_per_apply"]})
+    return c
+
+
+def run_ours(args):
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_1309_5571_b200 as lib
+    lib.load_library()
+
+    problem, cfg = make_problem(args.config)
+    k_max, reorth = cfg["k_max"], 1
+    plan = lib.Plan(problem, k_max=k_max, tol=1e-10, reorth=reorth, device=f"cuda:{local}")
+    st = plan.stats()
+    n = plan.n
+    V, W = plan.new_basis()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")
+    stream = torch.cuda.current_stream()
+
+    def restart_run():
+        plan.davidson_init(V, W, start_at_argmin_diag=True)
+        return 1
+
+    # ---- device-resident timing: W warm-up + K timed steps, per-step event pairs, L2 flushed between
+    def timed_run(steps, warmup, host_io):
+        k = restart_run()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        ks = []
+        l0 = 0
+        hx = torch.empty(n, dtype=torch.float64).pin_memory() if host_io else None
+        hw = torch.empty(n, dtype=torch.float64).pin_memory() if host_io else None
+        if host_io:
+            hx.copy_(V[0, :n])
+        for it in range(warmup + steps):
+            flush.zero_()
+            j = it - warmup
+            if j == 0:
+                l0 = plan.stats()["launches"]
+            if j >= 0:
+                ev[j][0].record(stream)
+                ks.append(k)
+            if host_io:   # newest basis vector in, projected vector out (pinned host buffers)
+                V[k - 1, :n].copy_(hx, non_blocking=True)
+            k_prev = k
+            k, lam, rho, conv = plan.davidson_step(V, W, k)
+            if host_io:
+                hw.copy_(W[k_prev - 1, :n], non_blocking=True)
+                stream.synchronize()
+            if j >= 0:
+                ev[j][1].record(stream)
+            if host_io and not conv:
+                hx.copy_(V[k - 1, :n])          # next step's input staged on the host (not timed as H2D yet)
+            if conv:
+                l0 -= plan.stats()["launches"]
+                k = restart_run()               # a new run's start vector is not part of the timed steps
+                l0 += plan.stats()["launches"]
+                if host_io:
+                    hx.copy_(V[0, :n])
+        torch.cuda.synchronize()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        return ms, ks, plan.stats()["launches"] - l0
+
+    sampler = ClockSampler(local)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    t0 = time.time()
+    ms, ks, gpu_launches = timed_run(args.steps, args.warmup, host_io=False)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t1 = time.time()
+    total_ms = sum(ms)
+    flop_step = [st["flop_per_apply"] + blas2_flop(n, k, 1 if k == k_max else k, reorth) for k in ks]
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * sum(flop_step) / (total_ms * 1e-3) / 1e9
+
+    # ---- end to end with host buffers
+    ms_e2e, ks_e, _ = timed_run(args.steps, args.warmup, host_io=True)
+    tot_e = sum(ms_e2e)
+    if dist is not None:
+        t = torch.tensor([tot_e], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tot_e = float(t.item())
+    flop_e = [st["flop_per_apply"] + blas2_flop(n, k, 1 if k == k_max else k, reorth) for k in ks_e]
+    e2e_val = world * sum(flop_e) / (tot_e * 1e-3) / 1e9
+
+    # ---- per-kernel device times of the same loop (library event pairs on the launching stream), warm L2
+    plan.set_timing(True)
+    k = restart_run()
+    kt = np.zeros(8); bytes_b2 = 0.0; nsteps_t = 0; t_b2 = 0.0
+    for it in range(args.warmup + args.steps):
+        kk = k
+        k, lam, rho, conv = plan.davidson_step(V, W, k)
+        if it >= args.warmup:
+            tm = plan.get_timing()
+            kt += tm; nsteps_t += 1
+            bytes_b2 += blas2_bytes(n, kk, 1 if kk == k_max else kk, reorth, kk == k_max)
+            t_b2 += tm[2] + tm[4] + tm[5] + tm[6] + tm[7]
+        if conv:
+            k = restart_run()
+    plan.set_timing(False)
+    clocks = sampler.stop(t0, time.time())      # sampled over the timed loops (device-resident, e2e, per-kernel)
+    kt /= max(nsteps_t, 1)
+    gemm_ms = kt[0] + kt[1]
+    # ---- apply alone, back to back (the H*psi GFLOP/s figure of BASELINE.json)
+    x = torch.randn(n, dtype=torch.float64, device=f"cuda:{local}"); y = torch.empty_like(x)
+    for _ in range(3):
+        plan.apply_H(x, y)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 50
+    e0.record(stream)
+    for _ in range(reps):
+        plan.apply_H(x, y)
+    e1.record(stream); torch.cuda.synchronize()
+    apply_ms = e0.elapsed_time(e1) / reps
+
+    # ---- roofline denominators: FP64 peak measured live (MEASURED_PEAKS.json has no FP64 entry), HBM from the file
+    dmma_peak = lib.dmrg_probe_fp64_peak(1, 3)
+    dfma_peak = lib.dmrg_probe_fp64_peak(0, 3)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.config, {}).get("grouped_gemm_dram_bytes_per_launch")
+    except Exception:
+        pass
+    achieved = st["flop_per_apply"] / (gemm_ms * 1e-3) / 1e12
+    roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (DMMA.8x8x4; 2 launches per step: stage 1 + stage 2)",
+                "achieved": achieved, "peak": max(dmma_peak, dfma_peak), "unit": "TFLOP/s",
+                "frac": achieved / max(dmma_peak, dfma_peak), "traffic": traffic,
+                "peak_source": "measured live: register-only DMMA.8x8x4 issue-rate probe (dmrg_probe_fp64_peak); "
+                               f"DFMA probe {dfma_peak:.1f}; nominal 148 SM x 128 FLOP/clk x 1.965 GHz = 37.2",
+                "flop_per_launch_pair": st["flop_per_apply"], "ms_per_launch_pair": gemm_ms}
+    blas2_gbs = bytes_b2 / max(t_b2 * 1e-3, 1e-12) / 1e9 / 1.0 if nsteps_t else None
+    if blas2_gbs is not None:
+        blas2_gbs = bytes_b2 / (t_b2 * 1e-3) / 1e9
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- oracle timed beside it (rank 0, N = 1 only): bounded sample
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        osteps = 20
+        gfl, oms, cores, _ = oracle_iteration_timer(problem, k_max, osteps, 2)
+        cpu_baseline = {"value": gfl, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": oms,
+                        "sample": f"{osteps} consecutive O-DAV iterations of {args.config} (k = 3..{2 + osteps}) from start e_argmin(D), numpy/BLAS threads = {cores}"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(args.config, cfg, n, st),
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n + 24,
+                    "ms_per_step": tot_e / args.steps},
+            "gpu_launches": int(gpu_launches),
+            "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "hpsi": {"gflops": st["flop_per_apply"] / (apply_ms * 1e-3) / 1e9, "ms": apply_ms,
+                     "frac_fp64_peak": st["flop_per_apply"] / (apply_ms * 1e-3) / 1e12 / max(dmma_peak, dfma_peak),
+                     "note": "dmrg_apply_H alone, back to back, warm L2"},
+            "davidson": {"iters_per_s": world * args.steps / (total_ms * 1e-3),
+                         "kernel_ms": {nm: float(v) for nm, v in zip(["apply_stage1", "apply_stage2", "vtw", "small_eig", "residual", "collapse", "orthogonalise", "append"], kt)},
+                         "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
+                         "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
+                         "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
+            "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -113,6 +113,9 @@ typedef struct {
     int64_t device_bytes;      /* everything the plan allocated on the device             */
     int32_t kernel_launches_per_apply;
     int32_t kernel_launches_per_step;  /* dmrg_davidson_step at reorth passes = options   */
+    int64_t flop_stage1, flop_stage2;  /* split of flop_per_apply over the two launches    */
+    int64_t launches;                  /* kernels launched by the hot-path entry points of
+                                          this plan since it was created (host-side count) */
 } dmrg_stats;
 
 typedef struct dmrg_plan *dmrg_handle_t;
@@ -206,8 +209,8 @@ int dmrg_probe_fp64_peak(int32_t kind, int32_t reps, double *tflops, void *cuda_
 int dmrg_probe_hbm_read(int64_t bytes, int32_t reps, double *gbs, void *cuda_stream);
 /* Per-kernel device time of the last dmrg_davidson_step when timing was enabled with
  * dmrg_set_timing(h, 1): ms[0] apply stage 1, [1] apply stage 2, [2] V^T w, [3] small eig,
- * [4] residual+precondition, [5] orthogonalise (all passes), [6] normalise/append,
- * [7] restart collapse.  HOST array of 8. */
+ * [4] residual+precondition, [5] restart collapse (0 unless k == k_max), [6] orthogonalise
+ * (all passes), [7] normalise/append.  HOST array of 8. */
 int dmrg_set_timing(dmrg_handle_t h, int32_t enable);
 int dmrg_get_timing(dmrg_handle_t h, double *ms8);
 

@@ -62,7 +62,8 @@ class Stats(C.Structure):
                 ("flop_per_apply", C.c_int64), ("operator_elems", C.c_int64), ("apply_bytes", C.c_int64),
                 ("stage1_units", C.c_int32), ("stage2_units", C.c_int32), ("stage2_split_tiles", C.c_int32),
                 ("pool_bytes", C.c_int64), ("workspace_bytes", C.c_int64), ("device_bytes", C.c_int64),
-                ("kernel_launches_per_apply", C.c_int32), ("kernel_launches_per_step", C.c_int32)]
+                ("kernel_launches_per_apply", C.c_int32), ("kernel_launches_per_step", C.c_int32),
+                ("flop_stage1", C.c_int64), ("flop_stage2", C.c_int64), ("launches", C.c_int64)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}

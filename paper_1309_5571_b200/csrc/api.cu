@@ -66,6 +66,7 @@ int dmrg_get_layout(dmrg_handle_t h, int64_t *n, int32_t *n_pairs, int32_t *left
 int dmrg_get_stats(dmrg_handle_t h, dmrg_stats *stats) {
     if (!h || !stats) return DMRG_E_INVALID_ARG;
     P(h)->stats.device_bytes = P(h)->device_bytes;
+    P(h)->stats.launches = P(h)->launches;
     *stats = P(h)->stats;
     return DMRG_OK;
 }

@@ -248,6 +248,7 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
     b.p[BASE_PART] = p->part;
     cudaEvent_t *ev = p->timing.enabled ? p->timing.ev : nullptr;
     if (ev) cudaEventRecord(ev[0], st);
+    p->launches += (p->n_units1 > 0 ? 1 : 0) + (p->n_units2 > 0 ? 1 : 0);
     cudaError_t e = launch_grouped_gemm(p->units1, p->n_units1, p->items1, b, p->counters, done_flag, st);
     if (ev) cudaEventRecord(ev[1], st);
     if (e == cudaSuccess) e = launch_grouped_gemm(p->units2, p->n_units2, p->items2, b, p->counters, done_flag, st);

@@ -100,6 +100,7 @@ struct Plan {
     // stats / misc
     dmrg_stats stats{};
     long long device_bytes = 0;
+    long long launches = 0;             // hot-path kernel launches (host-side count)
     std::string err;
     Timing timing;
     int sm_count = 148;

@@ -356,7 +356,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     std::vector<GemmItem> items1, items2;
     std::vector<TaskHost> tasks1, tasks2;
     std::vector<std::vector<GemmItem>> out_items(P);
-    long long tws_elems = 0, flops = 0;
+    long long tws_elems = 0, flops = 0, flops1 = 0;
     int n_gemms = 0;
     auto vec2 = [](long long off, int ld) { return (uint8_t)((off % 2 == 0 && ld % 2 == 0) ? 1 : 0); };
     for (const Record &r : recs) {
@@ -386,14 +386,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                 it1 = {xoff, B.off, (int)dk, B.ld, (int)dk, BASE_X, BASE_POOL, vec2(xoff, (int)dk), vec2(B.off, B.ld)};
                 t1 = {BASE_T, toff, ldt, (int)di, (int)dl, 0, 1};
                 it2 = {A.off, toff, A.ld, ldt, (int)di, BASE_POOL, BASE_T, vec2(A.off, A.ld), 1};
-                flops += f1;
+                flops += f1; flops1 += 2 * di * dk * dl;
             } else {
                 const int ldt = (int)round_up(dk, 2);
                 const long long toff = tws_elems; tws_elems += round_up(dj * ldt, 16);
                 it1 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
                 t1 = {BASE_T, toff, ldt, (int)dj, (int)dk, 0, 1};
                 it2 = {toff, B.off, ldt, B.ld, (int)dk, BASE_T, BASE_POOL, 1, vec2(B.off, B.ld)};
-                flops += f2;
+                flops += f2; flops1 += 2 * dj * di * dk;
             }
             t1.item_begin = (int)items1.size();
             items1.push_back(it1);
@@ -509,13 +509,13 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     // ---- stats
     dmrg_stats &s = p->stats;
     s.n = p->n; s.n_pairs = P; s.n_records = (int)recs.size(); s.n_gemms = n_gemms;
-    s.flop_per_apply = flops; s.operator_elems = bl.op_elems; s.apply_bytes = 8 * (bl.op_elems + 2 * p->n);
+    s.flop_per_apply = flops; s.flop_stage1 = flops1; s.flop_stage2 = flops - flops1; s.operator_elems = bl.op_elems; s.apply_bytes = 8 * (bl.op_elems + 2 * p->n);
     s.stage1_units = p->n_units1; s.stage2_units = p->n_units2; s.stage2_split_tiles = split_tiles2;
     s.pool_bytes = 8 * bl.pool_elems;
     s.workspace_bytes = 8 * (tws_elems + part_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
     s.device_bytes = p->device_bytes;
     s.kernel_launches_per_apply = (p->n_units1 > 0 ? 1 : 0) + 1;
-    s.kernel_launches_per_step = s.kernel_launches_per_apply + 5 + 2 * p->opt.reorth;
+    s.kernel_launches_per_step = s.kernel_launches_per_apply + 4 + 2 * p->opt.reorth;   // +2 on a restart step
     *out = p;
     return DMRG_OK;
 }
