@@ -142,7 +142,9 @@ int dmrg_set_small(dmrg_handle_t h, const double *B_host, void *stream) {
     const int km = p->opt.k_max;
     memset(p->state_host->B, 0, sizeof(p->state_host->B));
     for (int i = 0; i < km; i++) for (int j = 0; j < km; j++) p->state_host->B[i * KMAX + j] = B_host[i * km + j];
-    cudaError_t e = cudaMemcpyAsync(p->state->B, p->state_host->B, sizeof(p->state_host->B), cudaMemcpyHostToDevice, S(stream));
+    p->state_host->e_k = 0;   // the kept eigenvectors no longer belong to this B
+    cudaError_t e = cudaMemcpyAsync(&p->state->e_k, &p->state_host->e_k, sizeof(int), cudaMemcpyHostToDevice, S(stream));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->state->B, p->state_host->B, sizeof(p->state_host->B), cudaMemcpyHostToDevice, S(stream));
     if (e == cudaSuccess) e = cudaStreamSynchronize(S(stream));
     return e == cudaSuccess ? DMRG_OK : fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
 }

@@ -11,19 +11,20 @@
 // DFMA pipe gives 33.9).  Operands are staged through shared memory with a 3-stage cp.async
 // (LDGSTS) pipeline; padded rows (+4 doubles) make both fragment loads bank-conflict free.
 // Ragged edges and odd row strides are handled by zero-filling cp.async (src-size < cp-size).
+#include <cstdlib>
+#include <string>
 #include "internal.h"
 
 namespace dmrg {
 
 namespace {
 
-constexpr int STAGES = 3;
 constexpr int THREADS = 128;               // 4 warps, 2x2, warp tile 32x32
 constexpr int LDP = BK + 4;                // 20 doubles: rows land on distinct bank groups
 constexpr int LDQ = BN + 4;                // 68
 constexpr int P_STAGE = BM * LDP;          // doubles
 constexpr int Q_STAGE = BK * LDQ;
-constexpr int SMEM_BYTES = STAGES * (P_STAGE + Q_STAGE) * 8;
+constexpr int smem_bytes(int stages) { return stages * (P_STAGE + Q_STAGE) * 8; }
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *g, int src_bytes) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -44,13 +45,28 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 
 struct Cursor { int item; int k0; };   // position in the flattened k-tile sequence
 
-__device__ __forceinline__ void load_tiles(double *sP, double *sQ, const GemmItem &it, const BasePtrs &bases,
-                                           int m0, int n0, int M, int N, int k0, bool xvec, int tid) {
-    const double *P = bases.p[it.p_base] + it.p_off;
-    const double *Q = bases.p[it.q_base] + it.q_off;
+struct ItemRegs {          // the current item, resolved once per item (not once per k-tile)
+    const double *P, *Q;
+    int ldp, ldq, K;
+    bool pv, qv;
+};
+__device__ __forceinline__ ItemRegs resolve_item(const GemmItem *it, const BasePtrs &bases, bool xvec) {
+    ItemRegs r;
+    const long long po = it->p_off, qo = it->q_off;
+    const int pb = it->p_base, qb = it->q_base;
+    r.P = bases.p[pb] + po; r.Q = bases.p[qb] + qo;
+    r.ldp = it->ldp; r.ldq = it->ldq; r.K = it->K;
+    r.pv = it->p_vec2 && (pb != BASE_X || xvec);
+    r.qv = it->q_vec2 && (qb != BASE_X || xvec);
+    return r;
+}
+
+__device__ __forceinline__ void load_tiles(double *sP, double *sQ, const ItemRegs &it,
+                                           int m0, int n0, int M, int N, int k0, int tid) {
+    const double *P = it.P;
+    const double *Q = it.Q;
     const int K = it.K;
-    const bool pv = it.p_vec2 && (it.p_base != BASE_X || xvec);
-    const bool qv = it.q_vec2 && (it.q_base != BASE_X || xvec);
+    const bool pv = it.pv, qv = it.qv;
     // P tile: BM x BK
     if (pv) {
 #pragma unroll
@@ -93,7 +109,11 @@ __device__ __forceinline__ void load_tiles(double *sP, double *sQ, const GemmIte
     }
 }
 
-__global__ void __launch_bounds__(THREADS, 4)
+// MODE 0: every DMMA of the 64x64x16 tile is issued (padding multiplies zeros);
+// MODE 1: interior tiles take the same unpredicated path, edge tiles skip sub-tiles that hold only padding
+//         (8-granular in M, N; 4-granular in K).
+template <int STAGES, int MINB, int MODE>
+__global__ void __launch_bounds__(THREADS, MINB)
 grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restrict__ items, BasePtrs bases,
                     int *__restrict__ counters, const int *__restrict__ done_flag, int xvec, int yvec) {
     if (done_flag && *done_flag) return;
@@ -114,7 +134,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 #pragma unroll
         for (int j = 0; j < 4; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
 
-    // producer cursor: walk to kt_begin
+    // producer cursor: walk to kt_begin; the consumer follows the same sequence STAGES-1 tiles behind
     Cursor pc{0, 0};
     {
         int skip = u.kt_begin;
@@ -124,43 +144,72 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             skip -= nkt; pc.item++;
         }
     }
-    auto advance = [&](Cursor &c) {
-        c.k0 += BK;
-        if (c.k0 >= uitems[c.item].K) { c.item++; c.k0 = 0; }
-    };
-
     const int KT = u.kt_count;
+    ItemRegs cur{};
+    if (KT > 0) cur = resolve_item(uitems + pc.item, bases, xvec != 0);
+    Cursor cc = pc;
+    int ccK = cur.K;
+    auto produce = [&](int stage) {
+        load_tiles(sPbase + stage * P_STAGE, sQbase + stage * Q_STAGE, cur, u.m0, u.n0, u.M, u.N, pc.k0, tid);
+        pc.k0 += BK;
+        if (pc.k0 >= cur.K) {
+            pc.item++; pc.k0 = 0;
+            if (pc.item < u.item_count) cur = resolve_item(uitems + pc.item, bases, xvec != 0);
+        }
+    };
+    // sub-tiles of this warp that hold real rows / columns (8-granular): padding issues no DMMA
+    const int mi = min(max(u.M - (u.m0 + wm) + 7, 0) >> 3, 4);
+    const int nj = min(max(u.N - (u.n0 + wn) + 7, 0) >> 3, 4);
+    const bool full_warp_tile = (mi == 4 && nj == 4);
+
     int issued = 0;
 #pragma unroll
     for (int s = 0; s < STAGES - 1; s++) {
-        if (issued < KT) {
-            load_tiles(sPbase + s * P_STAGE, sQbase + s * Q_STAGE, uitems[pc.item], bases, u.m0, u.n0, u.M, u.N, pc.k0, xvec != 0, tid);
-            advance(pc); issued++;
-        }
+        if (issued < KT) { produce(s); issued++; }
         cp_async_commit();
     }
     for (int t = 0; t < KT; t++) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
-        if (issued < KT) {
-            const int s = issued % STAGES;
-            load_tiles(sPbase + s * P_STAGE, sQbase + s * Q_STAGE, uitems[pc.item], bases, u.m0, u.n0, u.M, u.N, pc.k0, xvec != 0, tid);
-            advance(pc); issued++;
-        }
+        if (issued < KT) { produce(issued % STAGES); issued++; }
         cp_async_commit();
+        const int nk4 = (min(ccK - cc.k0, BK) + 3) >> 2;    // k4-steps with real K in this tile
+        cc.k0 += BK;
+        if (cc.k0 >= ccK) {
+            cc.item++; cc.k0 = 0;
+            if (cc.item < u.item_count) ccK = uitems[cc.item].K;
+        }
         const double *pa = sPbase + (t % STAGES) * P_STAGE + (wm + g) * LDP + tg;
         const double *pb = sQbase + (t % STAGES) * Q_STAGE + tg * LDQ + wn + g;
+        if (MODE == 0 || (full_warp_tile && nk4 == BK / 4)) {
 #pragma unroll
-        for (int k4 = 0; k4 < BK / 4; k4++) {
-            double a[4], b[4];
+            for (int k4 = 0; k4 < BK / 4; k4++) {
+                double a[4], b[4];
 #pragma unroll
-            for (int i = 0; i < 4; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
+                for (int i = 0; i < 4; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
 #pragma unroll
-            for (int j = 0; j < 4; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
+                for (int j = 0; j < 4; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
 #pragma unroll
-            for (int i = 0; i < 4; i++)
+                for (int i = 0; i < 4; i++)
 #pragma unroll
-                for (int j = 0; j < 4; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                    for (int j = 0; j < 4; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            }
+        } else {
+            for (int k4 = 0; k4 < nk4; k4++) {
+                double a[4], b[4];
+#pragma unroll
+                for (int i = 0; i < 4; i++) a[i] = (i < mi) ? pa[i * 8 * LDP + k4 * 4] : 0.0;
+#pragma unroll
+                for (int j = 0; j < 4; j++) b[j] = (j < nj) ? pb[k4 * 4 * LDQ + j * 8] : 0.0;
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    if (i < mi) {
+#pragma unroll
+                        for (int j = 0; j < 4; j++)
+                            if (j < nj) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                    }
+                }
+            }
         }
     }
     cp_async_wait<0>();
@@ -226,8 +275,29 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 }  // namespace
 
+// kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
+typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, const int *, int, int);
+struct Variant { const char *name; gemm_fn fn; int smem; };
+static const Variant kVariants[] = {
+    {"s3b4m0", grouped_gemm_kernel<3, 4, 0>, smem_bytes(3)},   // default: measured best at cfg3 / cfg5a
+    {"s3b4m1", grouped_gemm_kernel<3, 4, 1>, smem_bytes(3)},
+    {"s3b3m1", grouped_gemm_kernel<3, 3, 1>, smem_bytes(3)},
+    {"s4b3m1", grouped_gemm_kernel<4, 3, 1>, smem_bytes(4)},
+    {"s4b2m1", grouped_gemm_kernel<4, 2, 1>, smem_bytes(4)},
+    {"s5b2m1", grouped_gemm_kernel<5, 2, 1>, smem_bytes(5)},
+    {"s4b2m0", grouped_gemm_kernel<4, 2, 0>, smem_bytes(4)},
+};
+static const Variant *g_variant = &kVariants[0];
+
 cudaError_t gemm_kernel_setup() {
-    return cudaFuncSetAttribute(grouped_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (const char *e = getenv("DMRG_GEMM_VARIANT"))
+        for (const Variant &v : kVariants)
+            if (std::string(v.name) == e) g_variant = &v;
+    for (const Variant &v : kVariants) {
+        cudaError_t err = cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem);
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
 }
 
 cudaError_t launch_grouped_gemm(const GemmUnit *units, int n_units, const GemmItem *items, const BasePtrs &bases,
@@ -235,7 +305,7 @@ cudaError_t launch_grouped_gemm(const GemmUnit *units, int n_units, const GemmIt
     if (n_units <= 0) return cudaSuccess;
     const int xvec = ((reinterpret_cast<uintptr_t>(bases.p[BASE_X]) & 15) == 0) ? 1 : 0;
     const int yvec = ((reinterpret_cast<uintptr_t>(bases.p[BASE_Y]) & 15) == 0) ? 1 : 0;
-    grouped_gemm_kernel<<<n_units, THREADS, SMEM_BYTES, st>>>(units, items, bases, counters, done_flag, xvec, yvec);
+    g_variant->fn<<<n_units, THREADS, g_variant->smem, st>>>(units, items, bases, counters, done_flag, xvec, yvec);
     return cudaGetLastError();
 }
 

@@ -60,6 +60,7 @@ struct DiagJob {              // D_seg[a,b] += c * da[a] * db[b]; null pointer =
 constexpr int KMAX = 32;
 struct DavState {
     double B[KMAX * KMAX];    // row-major, kept symmetric (A18)
+    double E[KMAX * KMAX];    // all eigenvectors of the last B (columns), warm start of the next small eig
     double y[KMAX];           // lowest eigenvector of B(0:k,0:k)
     double s[KMAX];           // Gram-Schmidt coefficients / scratch dot products
     double lambda, rho, rho2, tau2, nx2, x0n2;
@@ -68,7 +69,8 @@ struct DavState {
     int iters;                // applies performed (stops counting once done)
     int k_used;               // basis size in the last executed step
     int sweeps;               // Jacobi sweeps of the last small eig
-    int pad[3];
+    int e_k;                  // size of the B whose eigenvectors E holds (0 = invalid)
+    int pad[2];
 };
 
 struct Timing { bool enabled = false; cudaEvent_t ev[10]; double ms[8]; bool created = false; };

@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <map>
 #include "internal.h"
 
@@ -421,7 +422,10 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
             W += (long long)kt * ((t.M + BM - 1) / BM) * ((t.N + BN - 1) / BN);
         }
         const int kt_min = 8;
-        long long kt_unit = std::max<long long>(kt_min, (W + (long long)p->sm_count * 8 - 1) / ((long long)p->sm_count * 8));
+        // target: ~units_per_sm units per SM (default 8; DMRG_UNITS_PER_SM overrides for experiments)
+        long long ups = 8;
+        if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
+        long long kt_unit = std::max<long long>(kt_min, (W + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
         for (const TaskHost &t : tasks) {
             int kt = 0;
             for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
