@@ -208,11 +208,17 @@ int dmrg_probe_fp64_peak(int32_t kind, int32_t reps, double *tflops, void *cuda_
 /* Streams `bytes` of device memory (read-only sum) and returns GB/s (HOST). */
 int dmrg_probe_hbm_read(int64_t bytes, int32_t reps, double *gbs, void *cuda_stream);
 /* Per-kernel device time of the last dmrg_davidson_step when timing was enabled with
- * dmrg_set_timing(h, 1): ms[0] apply stage 1, [1] apply stage 2, [2] V^T w, [3] small eig,
+ * dmrg_set_timing(h, 1): ms[0] the apply (one grouped launch), [1] 0 (kept for layout), [2] V^T w, [3] small eig,
  * [4] residual+precondition, [5] restart collapse (0 unless k == k_max), [6] orthogonalise
  * (all passes), [7] normalise/append.  HOST array of 8. */
 int dmrg_set_timing(dmrg_handle_t h, int32_t enable);
 int dmrg_get_timing(dmrg_handle_t h, double *ms8);
+
+/* Diagnostics: per-work-unit timeline of the LAST dmrg_apply_H of this plan, recorded only when the
+ * plan was created with the environment variable DMRG_TRACE set (otherwise *n_units = 0).
+ * trace_host: HOST array of 4 * max_units uint64 -- per unit, in issue (ticket) order:
+ * start ns, end-of-main-loop ns, end ns (%globaltimer), SM id.  Synchronises the device. */
+int dmrg_get_unit_trace(dmrg_handle_t h, uint64_t *trace_host, int32_t max_units, int32_t *n_units);
 
 int dmrg_version(void);
 

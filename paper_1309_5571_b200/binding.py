@@ -23,7 +23,7 @@ EXPORTS = [
     "dmrg_plan_create", "dmrg_plan_destroy", "dmrg_get_layout", "dmrg_get_stats", "dmrg_get_diag",
     "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_get_small",
     "dmrg_set_small", "dmrg_ritz_vector", "dmrg_lowest_eigenpair", "dmrg_gemv_trans", "dmrg_gemv_sub",
-    "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_version",
+    "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
 ]
 
 
@@ -102,6 +102,7 @@ def load_library():
         "dmrg_probe_hbm_read": [i64, i32, pdbl, vp],
         "dmrg_set_timing": [vp, i32],
         "dmrg_get_timing": [vp, pdbl],
+        "dmrg_get_unit_trace": [vp, C.POINTER(C.c_uint64), i32, pi32],
         "dmrg_version": [],
     }
     for name, args in sig.items():
@@ -317,6 +318,15 @@ class Plan:
         ms = np.zeros(8)
         self._check(self._lib.dmrg_get_timing(self._h, ms.ctypes.data_as(C.POINTER(C.c_double))))
         return ms
+
+    def unit_trace(self):
+        """Diagnostics (plan created with DMRG_TRACE set): (n_units, 4) uint64 array of the last apply."""
+        st = self.stats()
+        cap = st["stage1_units"] + st["stage2_units"]
+        buf = np.zeros((max(cap, 1), 4), dtype=np.uint64)
+        nu = C.c_int32()
+        self._check(self._lib.dmrg_get_unit_trace(self._h, buf.ctypes.data_as(C.POINTER(C.c_uint64)), cap, C.byref(nu)))
+        return buf[: nu.value]
 
     def close(self):
         if getattr(self, "_h", None):

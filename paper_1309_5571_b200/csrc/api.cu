@@ -227,6 +227,19 @@ int dmrg_probe_hbm_read(int64_t bytes, int32_t reps, double *gbs, void *stream) 
     return probe_hbm(bytes, reps, gbs, S(stream));
 }
 
+int dmrg_get_unit_trace(dmrg_handle_t h, uint64_t *trace_host, int32_t max_units, int32_t *n_units) {
+    if (!h || !n_units) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    *n_units = 0;
+    if (!p->trace || !trace_host || max_units <= 0) return DMRG_OK;
+    const int nu = p->trace_units < max_units ? p->trace_units : max_units;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(trace_host, p->trace, 32 * (size_t)nu, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    *n_units = nu;
+    return DMRG_OK;
+}
+
 int dmrg_set_timing(dmrg_handle_t h, int32_t enable) {
     if (!h) return DMRG_E_INVALID_ARG;
     P(h)->timing.enabled = enable != 0;

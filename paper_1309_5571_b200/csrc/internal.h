@@ -20,6 +20,8 @@ struct GemmItem {
     int ldp, ldq, K;
     uint8_t p_base, q_base;
     uint8_t p_vec2, q_vec2;   // 16-byte loads legal (even offset, even ld)
+    int dep;                  // index of the T-block ready counter this item waits on (-1: reads no T)
+    int dep_need;             // tiles of that T block: the counter value that means "complete"
 };
 
 struct GemmUnit {
@@ -33,7 +35,12 @@ struct GemmUnit {
     int split_idx, n_split;
     uint8_t c_base, c_vec2;
     uint8_t pad[2];
+    int signal;               // T-block ready counter to bump once this tile of T is written (-1: none)
+    int cost;                 // scheduling weight (DMMA count + per-k-tile overhead)
 };
+
+// control words of one apply (device ints): ticket dispenser, finished count, then one ready counter per T block
+enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_DEP0 = 2 };
 
 struct BasePtrs { double *p[BASE_COUNT]; };
 
@@ -88,9 +95,12 @@ struct Plan {
     // device memory
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
     int *counters = nullptr;
-    GemmItem *items1 = nullptr, *items2 = nullptr;
-    GemmUnit *units1 = nullptr, *units2 = nullptr;
-    int n_units1 = 0, n_units2 = 0;
+    GemmItem *items = nullptr;          // stage-1 items, then stage-2 items
+    GemmUnit *units = nullptr;          // ticket order: stage-1 units, then stage-2 units
+    int n_units1 = 0, n_units2 = 0, n_deps = 0;
+    int *ctrl = nullptr;                // Ctrl layout, self-resetting
+    unsigned long long *trace = nullptr;   // optional per-unit timeline (4 words per unit), diagnostics
+    int trace_units = 0;
     // Davidson scratch
     DavState *state = nullptr;          // device
     DavState *state_host = nullptr;     // pinned
@@ -116,9 +126,6 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out);
 void plan_free(Plan *p);
 
 // gemm.cu
-cudaError_t launch_grouped_gemm(const GemmUnit *units, int n_units, const GemmItem *items,
-                                const BasePtrs &bases, int *counters, const int *done_flag,
-                                cudaStream_t st);
 cudaError_t gemm_kernel_setup();
 
 // davidson.cu

@@ -1,12 +1,13 @@
 // plan.cu -- host planner: admissible sector pairs, operation records grouped by output,
-// operator repacking, work units of the two grouped launches, diag(H_SB), workspaces.
+// operator repacking, work units of the grouped launch, diag(H_SB), workspaces.
 //
 // PAPER.md:L340-342 (operation records; "A, B are fixed" over the Davidson iteration),
 // L358-363 (Alg. 5 step 1: records and FLOP workload per output; all records of one output
 // stay with one owner -> no merging of outputs), L165-171 (Eq. 11).  The paper's stream
-// interleaving (Alg. 6-7) is replaced by two grouped launches: stage 1 forms the inner
-// product of every two-factor record, stage 2 forms each output tile as ONE product whose
-// K dimension is the concatenation over all records of that output (fixed order, no atomics).
+// interleaving (Alg. 6-7) is replaced by ONE grouped launch over ticket-ordered work units: stage-1
+// units form the inner product of every two-factor record, stage-2 units form each output tile as
+// ONE product whose K dimension is the concatenation over all records of that output (fixed
+// order, no atomics); a stage-2 unit waits on the "complete" counter of the T blocks it reads.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -76,7 +77,7 @@ struct PoolEntry { long long off; int rows, cols, ld; };
 struct FactorBlk { int src, dst, entry; };          // entry = pool index
 struct Term { bool A_id, B_id; std::vector<FactorBlk> A, B; };
 struct Record { int A, B, in_pair, out_pair; };      // pool entries or -1 (identity)
-struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; };
+struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; int out_pair; };
 
 inline long long round_up(long long v, long long a) { return (v + a - 1) / a * a; }
 
@@ -366,6 +367,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         const long long di = p->dimL[i], dk = p->dimR[k], dj = p->dimL[j], dl = p->dimR[l];
         const long long xoff = p->segOff[r.in_pair];
         GemmItem it2{};
+        int dep = -1;             // stage-1 task whose T block this record's stage-2 item reads
         if (r.B < 0) {            // A (x) I :  X'_jk += A X_ik
             const PoolEntry &A = bl.pool[r.A];
             it2 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
@@ -397,61 +399,105 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                 flops += f2; flops1 += 2 * dj * di * dk;
             }
             t1.item_begin = (int)items1.size();
+            t1.out_pair = r.out_pair;
+            it1.dep = -1; it1.dep_need = 0;
+            dep = (int)tasks1.size();
             items1.push_back(it1);
             tasks1.push_back(t1);
         }
+        it2.dep = dep;
+        it2.dep_need = dep < 0 ? 0 : ((tasks1[dep].M + BM - 1) / BM) * ((tasks1[dep].N + BN - 1) / BN);
         out_items[r.out_pair].push_back(it2);
     }
+    // inside one output the records that read X directly come first in the K order, so that a stage-2 unit
+    // starting at k = 0 has work before its first T block is complete (order fixed at plan time: deterministic)
+    for (auto &v : out_items)
+        std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return (a.dep < 0) > (b.dep < 0); });
     for (int op = 0; op < P; op++) {
         TaskHost t{};
         t.c_base = BASE_Y; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
         t.M = p->dimL[p->pairL[op]]; t.N = p->dimR[p->pairR[op]];
-        t.item_begin = (int)items2.size(); t.item_count = (int)out_items[op].size();
+        t.item_begin = (int)items2.size(); t.item_count = (int)out_items[op].size(); t.out_pair = op;
         for (const GemmItem &it : out_items[op]) items2.push_back(it);
         tasks2.push_back(t);   // outputs without any record are still zero-filled by the kernel
     }
 
-    // ---- work units: tiles x split of the concatenated K (fixed-order second-stage reduce)
+    // ---- work units: tiles x split of the concatenated K (fixed-order second-stage reduce).
+    // ONE launch runs both stages; units are handed out through a ticket counter in this order: stage-1 units
+    // grouped by output, outputs by descending cost -- so T blocks complete in the order stage 2 consumes them --
+    // then the stage-2 units in the same output order, so the last units of the launch are the small ones.
     long long part_elems = 0; int n_counters = 0; int split_tiles2 = 0;
-    auto make_units = [&](const std::vector<TaskHost> &tasks, const std::vector<GemmItem> &items,
-                          std::vector<GemmUnit> &units, int *split_tiles) {
-        long long W = 0;
-        for (const TaskHost &t : tasks) {
-            int kt = 0;
-            for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
-            W += (long long)kt * ((t.M + BM - 1) / BM) * ((t.N + BN - 1) / BN);
-        }
-        const int kt_min = 8;
-        // target: ~units_per_sm units per SM (default 8; DMRG_UNITS_PER_SM overrides for experiments)
-        long long ups = 8;
-        if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
-        long long kt_unit = std::max<long long>(kt_min, (W + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
-        for (const TaskHost &t : tasks) {
-            int kt = 0;
-            for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
+    auto ktiles = [&](const std::vector<GemmItem> &items, const TaskHost &t) {
+        int kt = 0;
+        for (int q = 0; q < t.item_count; q++) kt += (items[t.item_begin + q].K + BK - 1) / BK;
+        return kt;
+    };
+    auto ntiles = [](const TaskHost &t) { return (long long)((t.M + BM - 1) / BM) * ((t.N + BN - 1) / BN); };
+    long long Wtot = 0;
+    for (const TaskHost &t : tasks1) Wtot += (long long)ktiles(items1, t) * ntiles(t);
+    for (const TaskHost &t : tasks2) Wtot += (long long)ktiles(items2, t) * ntiles(t);
+    const int kt_min = 8;
+    // target: ~units_per_sm units per SM over the whole apply (DMRG_UNITS_PER_SM overrides for experiments)
+    long long ups = 16;
+    if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
+    const long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
+    std::vector<long long> out_cost(P, 0);
+    std::vector<int> unit_out, uo1, uo2;
+    auto make_units = [&](const std::vector<TaskHost> &tasks, const std::vector<GemmItem> &items, int item_shift,
+                          bool signals, std::vector<GemmUnit> &units, int *split_tiles) {
+        for (size_t ti = 0; ti < tasks.size(); ti++) {
+            const TaskHost &t = tasks[ti];
+            const int kt = ktiles(items, t);
             for (int m0 = 0; m0 < t.M; m0 += BM) for (int n0 = 0; n0 < t.N; n0 += BN) {
-                int ns = (int)std::max<long long>(1, (kt + kt_unit - 1) / kt_unit);
+                int ns = (int)std::max<long long>(1, (kt + kt_unit / 2) / kt_unit);
                 // never split below kt_min k-tiles per unit
                 while (ns > 1 && kt / ns < kt_min) ns--;
                 int tile_id = -1; long long poff = 0;
                 if (ns > 1) { tile_id = n_counters++; poff = part_elems; part_elems += (long long)ns * BM * BN; if (split_tiles) (*split_tiles)++; }
+                const int sub = ((std::min(BM, t.M - m0) + 7) / 8) * ((std::min(BN, t.N - n0) + 7) / 8);   // 8x8 sub-tiles with data
                 int base = kt / ns, rem = kt % ns, begin = 0;
-                for (int s = 0; s < ns; s++) {
+                for (int sp = 0; sp < ns; sp++) {
                     GemmUnit u{};
                     u.c_off = t.c_off; u.part_off = poff; u.ldc = t.ldc; u.M = t.M; u.N = t.N; u.m0 = m0; u.n0 = n0;
-                    u.item_begin = t.item_begin; u.item_count = t.item_count;
-                    u.kt_begin = begin; u.kt_count = base + (s < rem ? 1 : 0); begin += u.kt_count;
-                    u.tile_id = tile_id; u.split_idx = s; u.n_split = ns;
+                    u.item_begin = t.item_begin + item_shift; u.item_count = t.item_count;
+                    u.kt_begin = begin; u.kt_count = base + (sp < rem ? 1 : 0); begin += u.kt_count;
+                    u.tile_id = tile_id; u.split_idx = sp; u.n_split = ns;
                     u.c_base = t.c_base; u.c_vec2 = vec2(t.c_off, t.ldc);
+                    u.signal = signals ? (int)ti : -1;
+                    u.cost = u.kt_count * (4 * sub + 64);
+                    out_cost[t.out_pair] += u.cost;
                     units.push_back(u);
+                    unit_out.push_back(t.out_pair);
                 }
             }
         }
-        std::stable_sort(units.begin(), units.end(), [](const GemmUnit &a, const GemmUnit &b) { return a.kt_count > b.kt_count; });
+    };
+    auto order_units = [&](std::vector<GemmUnit> &units, std::vector<int> &uo) {
+        std::vector<int> idx(units.size());
+        for (size_t q = 0; q < idx.size(); q++) idx[q] = (int)q;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+            if (uo[a] != uo[b]) {
+                if (out_cost[uo[a]] != out_cost[uo[b]]) return out_cost[uo[a]] > out_cost[uo[b]];
+                return uo[a] < uo[b];
+            }
+            return units[a].cost > units[b].cost;
+        });
+        std::vector<GemmUnit> v; v.reserve(units.size());
+        for (int q : idx) v.push_back(units[q]);
+        units.swap(v);
     };
     std::vector<GemmUnit> units1, units2;
-    make_units(tasks1, items1, units1, nullptr);
-    make_units(tasks2, items2, units2, &split_tiles2);
+    make_units(tasks1, items1, 0, true, units1, nullptr);
+    uo1.swap(unit_out);
+    make_units(tasks2, items2, (int)items1.size(), false, units2, &split_tiles2);
+    uo2.swap(unit_out);
+    order_units(units1, uo1);     // out_cost now holds stage 1 + stage 2 of every output
+    order_units(units2, uo2);
+    std::vector<GemmUnit> units(units1);
+    units.insert(units.end(), units2.begin(), units2.end());
+    std::vector<GemmItem> items(items1);
+    items.insert(items.end(), items2.begin(), items2.end());
+    p->n_deps = (int)tasks1.size();
 
     // ---- device allocations
     CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
@@ -459,18 +505,21 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->part, part_elems));
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
-    CUDA_TRY(p, dev_alloc(p, &p->items1, (long long)items1.size()));
-    CUDA_TRY(p, dev_alloc(p, &p->items2, (long long)items2.size()));
-    CUDA_TRY(p, dev_alloc(p, &p->units1, (long long)units1.size()));
-    CUDA_TRY(p, dev_alloc(p, &p->units2, (long long)units2.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + p->n_deps));
+    CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + p->n_deps)));
+    if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
+        p->trace_units = (int)units.size();
+        CUDA_TRY(p, dev_alloc(p, &p->trace, 4LL * std::max<long long>(p->trace_units, 1)));
+        CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
+    }
     CUDA_TRY(p, cudaMemset(p->pool, 0, sizeof(double) * std::max<long long>(bl.pool_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->tws, 0, sizeof(double) * std::max<long long>(tws_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->counters, 0, sizeof(int) * std::max(n_counters, 1)));
     CUDA_TRY(p, cudaMemset(p->D, 0, sizeof(double) * p->n));
-    if (!items1.empty()) CUDA_TRY(p, cudaMemcpy(p->items1, items1.data(), items1.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
-    if (!items2.empty()) CUDA_TRY(p, cudaMemcpy(p->items2, items2.data(), items2.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
-    if (!units1.empty()) CUDA_TRY(p, cudaMemcpy(p->units1, units1.data(), units1.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
-    if (!units2.empty()) CUDA_TRY(p, cudaMemcpy(p->units2, units2.data(), units2.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
+    if (!items.empty()) CUDA_TRY(p, cudaMemcpy(p->items, items.data(), items.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
+    if (!units.empty()) CUDA_TRY(p, cudaMemcpy(p->units, units.data(), units.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
     p->n_units1 = (int)units1.size(); p->n_units2 = (int)units2.size();
 
     // ---- repack the operators (scaled / transposed / aligned), once
@@ -518,7 +567,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     s.pool_bytes = 8 * bl.pool_elems;
     s.workspace_bytes = 8 * (tws_elems + part_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
     s.device_bytes = p->device_bytes;
-    s.kernel_launches_per_apply = (p->n_units1 > 0 ? 1 : 0) + 1;
+    s.kernel_launches_per_apply = 1;
     s.kernel_launches_per_step = s.kernel_launches_per_apply + 4 + 2 * p->opt.reorth;   // +2 on a restart step
     *out = p;
     return DMRG_OK;
@@ -527,7 +576,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
 void plan_free(Plan *p) {
     if (!p) return;
     cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
-    cudaFree(p->items1); cudaFree(p->items2); cudaFree(p->units1); cudaFree(p->units2);
+    cudaFree(p->items); cudaFree(p->units); cudaFree(p->ctrl); cudaFree(p->trace);
     cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
     cudaFree(p->Vown); cudaFree(p->Wown);
