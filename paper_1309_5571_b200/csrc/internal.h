@@ -129,6 +129,7 @@ void plan_free(Plan *p);
 cudaError_t gemm_kernel_setup();
 
 // davidson.cu
+void dav_setup(Plan *p);
 int dav_init(Plan *p, const double *x0, int argmin_start, double *V, double *W, long long ldv, cudaStream_t st);
 int dav_enqueue_step(Plan *p, double *V, double *W, long long ldv, int k, cudaStream_t st, int *k_next);
 int dav_ritz(Plan *p, const double *V, long long ldv, int k, double *x_out, cudaStream_t st);

@@ -545,7 +545,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, cudaGetLastError());
 
     // ---- Davidson scratch
-    p->vec_grid = (int)std::max<long long>(1, std::min<long long>((long long)p->sm_count * 4, (p->n + 511) / 512));
+    p->vec_grid = p->sm_count * 8;      // capacity of the partials buffer; each kernel launches one wave of its own (davidson.cu)
     CUDA_TRY(p, dev_alloc(p, &p->state, 1));
     CUDA_TRY(p, cudaMemset(p->state, 0, sizeof(DavState)));
     CUDA_TRY(p, cudaMallocHost((void **)&p->state_host, sizeof(DavState)));
@@ -557,6 +557,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->vec_counter, 4));
     CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
     CUDA_TRY(p, gemm_kernel_setup());
+    dav_setup(p);
     CUDA_TRY(p, cudaDeviceSynchronize());
 
     // ---- stats
