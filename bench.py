@@ -9,7 +9,7 @@ spin-1/2, Delta=0.5, synthetic blocks m=2048 per side, Sz sectors -16..16, targe
 and synthetic (DESIGN.md "Input recipe").
 
 A step = one call of Alg. 3 = one pass of the whole hot path: the projection
-W(:,k) = H_SB V(:,k) (two grouped DMMA launches) plus every BLAS-2 row of SURVEY 8(a) (V^T w, small
+W(:,k) = H_SB V(:,k) (one grouped DMMA launch running both GEMM stages) plus every BLAS-2 row of SURVEY 8(a) (V^T w, small
 eig, residual + preconditioner, Gram-Schmidt, normalise/append, restart collapse when due), through
 the C ABI (dmrg_davidson_step), basis size cycling 1..k_max as in a real run.
 
@@ -18,7 +18,9 @@ value   = algorithmic FP64 GFLOP/s of the whole step (A24 FLOP of the apply + BL
 e2e     = same metric with host buffers: every step copies the newest basis vector host->device from
           pinned memory and the projected vector W(:,k) device->host (the per-iteration crossing of the
           paper's hybrid scheme: H2D of the input, D2H of the output, Alg. 7).
-roofline= the grouped DMMA kernel (both launches of a step) against the FP64 DMMA peak measured live.
+roofline= the grouped DMMA kernel (one launch per step) against the FP64 DMMA peak measured live.
+davidson_hbm = the BLAS-2 kernels timed inside running steps at config 5b (n ~ 1.5e7: V, W >> L2) against the
+          measured HBM copy bandwidth (the >= 75 % judgement is taken where V >> L2).
 cpu_baseline / --impl reference = the oracle's O-DAV iteration (oracle/, numpy) on the host cores.
 """
 from __future__ import annotations
@@ -152,6 +154,47 @@ def workload_config(name, cfg, n, stats):
     if stats:
         c.update({"n_records": stats["n_records"], "n_gemms": stats["n_gemms"], "flop_per_apply": stats["flop_per_apply"]})
     return c
+
+
+def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
+    """BLAS-2 kernels inside running Davidson steps at a config whose basis is far larger than L2."""
+    import torch
+    problem, cfg = make_problem(name)
+    k_max = cfg["k_max"]
+    plan = lib.Plan(problem, k_max=k_max, tol=1e-10, device=device)
+    n = plan.n
+    V, W = plan.new_basis()
+    plan.davidson_init(V, W, start_at_argmin_diag=True)
+    plan.set_timing(True)
+    k = 1
+    acc = {"vtw": [0.0, 0.0], "residual": [0.0, 0.0], "orthogonalise": [0.0, 0.0], "append": [0.0, 0.0]}
+    t_apply = []
+    for it in range(steps):
+        kk = k
+        k, lam, rho, conv = plan.davidson_step(V, W, k)
+        tm = plan.get_timing()
+        if it >= 3 and kk < k_max:
+            ke = kk
+            for nm, b, ms in (("vtw", 8.0 * n * (kk + 1), tm[2]), ("residual", 8.0 * n * 2 * kk + 16.0 * n, tm[4]),
+                              ("orthogonalise", 2 * 8.0 * n * (ke + 1) + 8.0 * n, tm[6]), ("append", 16.0 * n, tm[7])):
+                acc[nm][0] += b; acc[nm][1] += ms
+            t_apply.append(tm[0] + tm[1])
+        if conv:
+            break
+    st = plan.stats()
+    out = {"workload": f"{name}: {cfg['kind']} m={cfg['m']} per side, n={n}, k = 4..{k_max - 1}, V and W {2 * V.numel() * 8 / 1e9:.1f} GB",
+           "kernels_gbs": {nm: v[0] / (v[1] * 1e-3) / 1e9 for nm, v in acc.items() if v[1] > 0},
+           "hbm_peak_gbs": hbm_peak}
+    tot_b = sum(v[0] for v in acc.values()); tot_ms = sum(v[1] for v in acc.values())
+    out["blas2_gbs"] = tot_b / (tot_ms * 1e-3) / 1e9
+    out["blas2_frac_hbm"] = out["blas2_gbs"] / hbm_peak
+    out["kernels_frac_hbm"] = {nm: g / hbm_peak for nm, g in out["kernels_gbs"].items()}
+    out["apply_tflops"] = st["flop_per_apply"] / (sum(t_apply) / len(t_apply) * 1e-3) / 1e12
+    out["device_bytes"] = st["device_bytes"] + 2 * V.numel() * 8
+    out["peak_allocated_bytes"] = int(torch.cuda.max_memory_allocated())
+    plan.close()
+    del V, W
+    return out
 
 
 def run_ours(args):
@@ -296,12 +339,12 @@ def run_ours(args):
     except Exception:
         pass
     achieved = st["flop_per_apply"] / (gemm_ms * 1e-3) / 1e12
-    roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (DMMA.8x8x4; 2 launches per step: stage 1 + stage 2)",
+    roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (DMMA.8x8x4; 1 launch per step: stage-1 and stage-2 units in ticket order)",
                 "achieved": achieved, "peak": max(dmma_peak, dfma_peak), "unit": "TFLOP/s",
                 "frac": achieved / max(dmma_peak, dfma_peak), "traffic": traffic,
                 "peak_source": "measured live: register-only DMMA.8x8x4 issue-rate probe (dmrg_probe_fp64_peak); "
                                f"DFMA probe {dfma_peak:.1f}; nominal 148 SM x 128 FLOP/clk x 1.965 GHz = 37.2",
-                "flop_per_launch_pair": st["flop_per_apply"], "ms_per_launch_pair": gemm_ms}
+                "flop_per_launch": st["flop_per_apply"], "ms_per_launch": gemm_ms}
     blas2_gbs = bytes_b2 / max(t_b2 * 1e-3, 1e-12) / 1e9 / 1.0 if nsteps_t else None
     if blas2_gbs is not None:
         blas2_gbs = bytes_b2 / (t_b2 * 1e-3) / 1e9
@@ -310,6 +353,14 @@ def run_ours(args):
         if dist is not None:
             dist.destroy_process_group()
         return
+
+    dav_large = None
+    if world == 1 and not args.no_large:
+        try:
+            dav_large = davidson_hbm_probe(lib, f"cuda:{local}", hbm_peak)
+            dav_large["apply_frac_fp64_peak"] = dav_large["apply_tflops"] / max(dmma_peak, dfma_peak)
+        except Exception as e:   # the headline numbers above do not depend on this extra config
+            dav_large = {"error": repr(e)}
 
     # ---- oracle timed beside it (rank 0, N = 1 only): bounded sample
     cpu_baseline = None
@@ -331,10 +382,11 @@ def run_ours(args):
                      "frac_fp64_peak": st["flop_per_apply"] / (apply_ms * 1e-3) / 1e12 / max(dmma_peak, dfma_peak),
                      "note": "dmrg_apply_H alone, back to back, warm L2"},
             "davidson": {"iters_per_s": world * args.steps / (total_ms * 1e-3),
-                         "kernel_ms": {nm: float(v) for nm, v in zip(["apply_stage1", "apply_stage2", "vtw", "small_eig", "residual", "collapse", "orthogonalise", "append"], kt)},
+                         "kernel_ms": {nm: float(v) for nm, v in zip(["apply", "apply_unused", "vtw", "small_eig", "residual", "collapse", "orthogonalise", "append"], kt)},
                          "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
                          "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
                          "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
+            "davidson_hbm": dav_large,
             "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -349,6 +401,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-large", action="store_true", help="skip the config-5b Davidson HBM measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
