@@ -197,6 +197,19 @@ def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
     return out
 
 
+def job_throughput(local_ms: float, local_flop: float, world: int, dist=None, device="cpu"):
+    """Whole-job metric of N replicas (replicas only, no data-path collective): the time of the
+    job is the MAX over ranks of the device-timed region, the work is the sum over ranks.  Returns (max_ms, GFLOP/s)."""
+    if dist is None or world == 1:
+        return local_ms, local_flop / (local_ms * 1e-3) / 1e9
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    f = torch.tensor([local_flop], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(f, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(f.item()) / (float(t.item()) * 1e-3) / 1e9
+
+
 def run_ours(args):
     import torch
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -277,21 +290,13 @@ def run_ours(args):
     t1 = time.time()
     total_ms = sum(ms)
     flop_step = [st["flop_per_apply"] + blas2_flop(n, k, 1 if k == k_max else k, reorth) for k in ks]
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * sum(flop_step) / (total_ms * 1e-3) / 1e9
+    total_ms, value = job_throughput(total_ms, sum(flop_step), world, dist, f"cuda:{local}")
 
     # ---- end to end with host buffers
     ms_e2e, ks_e, _ = timed_run(args.steps, args.warmup, host_io=True)
     tot_e = sum(ms_e2e)
-    if dist is not None:
-        t = torch.tensor([tot_e], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tot_e = float(t.item())
     flop_e = [st["flop_per_apply"] + blas2_flop(n, k, 1 if k == k_max else k, reorth) for k in ks_e]
-    e2e_val = world * sum(flop_e) / (tot_e * 1e-3) / 1e9
+    tot_e, e2e_val = job_throughput(tot_e, sum(flop_e), world, dist, f"cuda:{local}")
 
     # ---- per-kernel device times of the same loop (library event pairs on the launching stream), warm L2
     plan.set_timing(True)

@@ -438,7 +438,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     for (const TaskHost &t : tasks2) Wtot += (long long)ktiles(items2, t) * ntiles(t);
     const int kt_min = 8;
     // target: ~units_per_sm units per SM over the whole apply (DMRG_UNITS_PER_SM overrides for experiments)
-    long long ups = 16;
+    // (measured: 16 is best at cfg 3 / 5a, ~280 k-tile units per SM; 24 at the 4096 sweep, 2200 per SM; flat beyond)
+    long long ups = (Wtot / std::max(p->sm_count, 1) < 1000) ? 16 : 24;
     if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
     const long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
     std::vector<long long> out_cost(P, 0);
