@@ -329,8 +329,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             }
         }
     }
-    // publish: this tile of a T block is complete (release: every thread's stores, then the counter)
-    __threadfence();
+    // publish: this tile of a T block is complete (release: every thread's stores, then the counter);
+    // units that publish nothing skip the fence
+    if (writes_c && u.signal >= 0) __threadfence();
     __syncthreads();
     if (tid == 0) {
         if (writes_c && u.signal >= 0) atomicAdd(&ctrl[CTRL_DEP0 + u.signal], 1);
