@@ -436,7 +436,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     long long Wtot = 0;
     for (const TaskHost &t : tasks1) Wtot += (long long)ktiles(items1, t) * ntiles(t);
     for (const TaskHost &t : tasks2) Wtot += (long long)ktiles(items2, t) * ntiles(t);
-    const int kt_min = 8;
+    const int kt_min = 6;
     // target: ~units_per_sm units per SM over the whole apply (DMRG_UNITS_PER_SM overrides for experiments)
     // (measured: 16 is best at cfg 3 / 5a, ~280 k-tile units per SM; 24 at the 4096 sweep, 2200 per SM; flat beyond)
     long long ups = (Wtot / std::max(p->sm_count, 1) < 1000) ? 16 : 24;
@@ -444,13 +444,36 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     const long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
     std::vector<long long> out_cost(P, 0);
     std::vector<int> unit_out, uo1, uo2;
+    // "guided" unit size for stage 2: the outputs that come last in ticket order get smaller K slices (the drain of
+    // the launch lasts about one unit, so the last units should be short): scale = clamp(tail * (1 - f), lo, 1) with
+    // f = fraction of the stage-2 k-tile volume that precedes the output in ticket order
+    std::vector<double> unit_scale(P, 1.0);
+    {
+        double tail = 3.0, lo = 0.5;     // measured: within 2 % of each other at cfg 3 / 5a / 4096; 3.0 / 0.5 marginally best
+        if (const char *e = getenv("DMRG_TAIL")) tail = atof(e);
+        if (const char *e = getenv("DMRG_TAIL_LO")) lo = atof(e);
+        std::vector<long long> vol(P, 0); long long tot2 = 0;
+        std::vector<long long> volall(P, 0);
+        for (int op = 0; op < P; op++) { vol[op] = (long long)ktiles(items2, tasks2[op]) * ntiles(tasks2[op]); tot2 += vol[op]; volall[op] = vol[op]; }
+        for (const TaskHost &t : tasks1) volall[t.out_pair] += (long long)ktiles(items1, t) * ntiles(t);
+        std::vector<int> ord(P);
+        for (int op = 0; op < P; op++) ord[op] = op;
+        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return volall[a] > volall[b]; });
+        long long before = 0;
+        for (int op : ord) {
+            const double f = tot2 > 0 ? (double)before / (double)tot2 : 0.0;
+            if (tail > 0) unit_scale[op] = std::min(1.0, std::max(lo, tail * (1.0 - f)));
+            before += vol[op];
+        }
+    }
     auto make_units = [&](const std::vector<TaskHost> &tasks, const std::vector<GemmItem> &items, int item_shift,
                           bool signals, std::vector<GemmUnit> &units, int *split_tiles) {
         for (size_t ti = 0; ti < tasks.size(); ti++) {
             const TaskHost &t = tasks[ti];
             const int kt = ktiles(items, t);
+            const long long kt_unit_t = signals ? kt_unit : std::max<long long>(kt_min, (long long)(kt_unit * unit_scale[t.out_pair]));
             for (int m0 = 0; m0 < t.M; m0 += BM) for (int n0 = 0; n0 < t.N; n0 += BN) {
-                int ns = (int)std::max<long long>(1, (kt + kt_unit / 2) / kt_unit);
+                int ns = (int)std::max<long long>(1, (kt + kt_unit_t / 2) / kt_unit_t);
                 // never split below kt_min k-tiles per unit
                 while (ns > 1 && kt / ns < kt_min) ns--;
                 int tile_id = -1; long long poff = 0;
