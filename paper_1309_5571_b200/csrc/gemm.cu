@@ -185,15 +185,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     const int colb8 = (u.n0 + (tid & 63) < u.N) ? 8 : 0;
 
     // producer cursor: walk to kt_begin; the consumer follows the same sequence STAGES-1 tiles behind
-    int p_item = 0, p_k0 = 0;
-    {
-        int skip = u.kt_begin;
-        while (p_item < u.item_count) {
-            const int nkt = (uitems[p_item].K + BK - 1) / BK;
-            if (skip < nkt) { p_k0 = skip * BK; break; }
-            skip -= nkt; p_item++;
-        }
-    }
+    int p_item = u.item0, p_k0 = u.k00;      // resolved by the planner
     const int KT = u.kt_count;
     Producer pr{};
     if (KT > 0) begin_item(pr, uitems + p_item, bases, xvec != 0, u.m0, u.n0, p_k0, tid, ctrl);

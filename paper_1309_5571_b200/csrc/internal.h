@@ -37,6 +37,7 @@ struct GemmUnit {
     uint8_t pad[2];
     int signal;               // T-block ready counter to bump once this tile of T is written (-1: none)
     int cost;                 // scheduling weight (DMMA count + per-k-tile overhead)
+    int item0, k00;           // where kt_begin falls: item index inside the unit's item list and k offset inside that item
 };
 
 // control words of one apply (device ints): ticket dispenser, finished count, then one ready counter per T block

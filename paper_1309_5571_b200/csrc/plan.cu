@@ -489,6 +489,15 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                     u.c_base = t.c_base; u.c_vec2 = vec2(t.c_off, t.ldc);
                     u.signal = signals ? (int)ti : -1;
                     u.cost = u.kt_count * (4 * sub + 64);
+                    {   // resolve kt_begin to (item, k offset) here, so that the kernel does not walk the item list
+                        int skip = u.kt_begin, q = 0;
+                        for (; q < t.item_count; q++) {
+                            const int nkt = (items[t.item_begin + q].K + BK - 1) / BK;
+                            if (skip < nkt) break;
+                            skip -= nkt;
+                        }
+                        u.item0 = q; u.k00 = skip * BK;
+                    }
                     out_cost[t.out_pair] += u.cost;
                     units.push_back(u);
                     unit_out.push_back(t.out_pair);
