@@ -18,7 +18,8 @@
 // DFMA pipe gives 33.9).  Operands are staged through shared memory with a 3-stage cp.async
 // (LDGSTS) pipeline whose per-thread source pointers are bumped, not recomputed, per k-tile;
 // padded rows (+4 doubles) make both fragment loads bank-conflict free.  Ragged edges and odd row
-// strides are handled by zero-filling cp.async (src-size < cp-size).
+// strides are handled by zero-filling cp.async (src-size < cp-size); a warp whose 32x32 tile holds data only in
+// its first 16 rows and/or columns runs a 2x4, 4x2 or 2x2 block of DMMA tiles instead of 4x4 (no predicates).
 #include <cstdlib>
 #include <string>
 #include "internal.h"
@@ -144,8 +145,27 @@ __device__ __forceinline__ void produce_tile(Producer &pr, double *sP, double *s
     pr.k0 = k0 + BK;
 }
 
+// One k-tile of the warp tile restricted to its first MI x NJ sub-tiles (compile-time bounds: no predicates).
+template <int MI, int NJ>
+__device__ __forceinline__ void mma_ktile(double (&acc)[4][4][2], const double *pa, const double *pb) {
+#pragma unroll
+    for (int k4 = 0; k4 < BK / 4; k4++) {
+        double a[MI], b[NJ];
+#pragma unroll
+        for (int i = 0; i < MI; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
+#pragma unroll
+        for (int j = 0; j < NJ; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
+#pragma unroll
+        for (int i = 0; i < MI; i++)
+#pragma unroll
+            for (int j = 0; j < NJ; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+    }
+}
+
 // MODE 0: every DMMA of the 64x64x16 tile is issued (padding multiplies zeros);
-// MODE 1: sub-tiles that hold only padding are skipped (8-granular in M, N; 4-granular in K).
+// MODE 1: sub-tiles that hold only padding are skipped (8-granular in M, N; 4-granular in K);
+// MODE 2: warp tiles whose data fits in the first 2 sub-tile rows / columns run a 2x4, 4x2 or 2x2 DMMA block
+//         (16-granular, no predicates), empty warp tiles run nothing.
 template <int STAGES, int MINB, int MODE>
 __global__ void __launch_bounds__(THREADS, MINB)
 grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restrict__ items, BasePtrs bases,
@@ -221,7 +241,12 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         }
         const double *pa = sPbase + (t % STAGES) * P_STAGE + (wm + g) * LDP + tg;
         const double *pb = sQbase + (t % STAGES) * Q_STAGE + tg * LDQ + wn + g;
-        if (MODE == 0 || (full_warp_tile && nk4 == BK / 4)) {
+        if (MODE == 2) {
+            if (mi > 2 && nj > 2) mma_ktile<4, 4>(acc, pa, pb);
+            else if (mi > 2 && nj > 0) mma_ktile<4, 2>(acc, pa, pb);
+            else if (mi > 0 && nj > 2) mma_ktile<2, 4>(acc, pa, pb);
+            else if (mi > 0 && nj > 0) mma_ktile<2, 2>(acc, pa, pb);
+        } else if (MODE == 0 || (full_warp_tile && nk4 == BK / 4)) {
 #pragma unroll
             for (int k4 = 0; k4 < BK / 4; k4++) {
                 double a[4], b[4];
@@ -347,10 +372,10 @@ typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int
                         unsigned long long *);
 struct Variant { const char *name; gemm_fn fn; int smem; };
 static const Variant kVariants[] = {
-    {"s3b4m0", grouped_gemm_kernel<3, 4, 0>, smem_bytes(3)},   // default: measured best at cfg3 / cfg5a
+    {"s3b4m2", grouped_gemm_kernel<3, 4, 2>, smem_bytes(3)},   // default: measured best at cfg3 / 5a / 5b / 4096 sweep
+    {"s3b4m0", grouped_gemm_kernel<3, 4, 0>, smem_bytes(3)},
     {"s3b4m1", grouped_gemm_kernel<3, 4, 1>, smem_bytes(3)},
-    {"s4b3m0", grouped_gemm_kernel<4, 3, 0>, smem_bytes(4)},
-    {"s4b3m1", grouped_gemm_kernel<4, 3, 1>, smem_bytes(4)},
+    {"s4b3m2", grouped_gemm_kernel<4, 3, 2>, smem_bytes(4)},
 };
 static const Variant *g_variant = &kVariants[0];
 
