@@ -229,3 +229,32 @@ def test_not_converged_and_breakdown_codes(lib):
         plan.davidson_step(V, W, 1)
     assert e.value.code == lib.DMRG_E_NUMERIC
     plan.close()
+
+
+def test_small_eig_fast_path_equals_jacobi_fallback():
+    """Line 4 has two implementations in one kernel: the arrowhead secular solve (warm start, k >= 5) and the Jacobi
+    sweeps it falls back to.  DMRG_EIG_FAST is read once per process, so each mode runs in its own process; the
+    lambda / ||r|| trajectories from the deterministic start must agree to rounding."""
+    import json, os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys, json; sys.path.insert(0, %r)\n"
+        "import torch, paper_1309_5571_b200 as lib\n"
+        "from dmrg_inputs import make_config\n"
+        "plan = lib.Plan(make_config('cfg2', 160), k_max=16, tol=1e-10)\n"
+        "V, W = plan.new_basis(); plan.davidson_init(V, W, start_at_argmin_diag=True)\n"
+        "k = 1; out = []\n"
+        "for it in range(45):\n"
+        "    k, lam, rho, conv = plan.davidson_step(V, W, k); out.append((lam, rho))\n"
+        "    if conv: break\n"
+        "print(json.dumps(out))\n") % root
+    runs = []
+    for mode in ("1", "0"):
+        r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600,
+                           env=dict(os.environ, DMRG_EIG_FAST=mode))
+        assert r.returncode == 0, r.stderr[-2000:]
+        runs.append(np.array(json.loads(r.stdout.strip().splitlines()[-1])))
+    fast, jac = runs
+    assert fast.shape == jac.shape and len(fast) >= 20
+    assert np.max(np.abs(fast[:, 0] - jac[:, 0])) <= 1e-10
+    assert np.max(np.abs(fast[:, 1] - jac[:, 1]) / (1e-12 + np.abs(jac[:, 1]))) <= 1e-5
