@@ -48,12 +48,15 @@ def blas2_flop(n: int, k: int, k_eff: int, reorth: int) -> float:
 
 
 def blas2_bytes(n: int, k: int, k_eff: int, reorth: int, restart: bool) -> float:
-    """Algorithmic bytes of the BLAS-2 rows of one step."""
+    """Algorithmic bytes of the BLAS-2 rows of one step (with the V^T t of the first Gram-Schmidt pass
+    sharing the residual pass over V: 8 n (4k + 7) per step instead of 8 n (5k + 8))."""
     b = 8.0 * n * (k + 1)                       # a3  V^T w
     b += 8.0 * n * (2 * k) + 16.0 * n           # a5-a7 fused: V, W, D read, t written
     if restart:
         b += 16.0 * n + 32.0 * n                # x, Wy written; collapse reads them and writes V0, W0
-    b += reorth * (8.0 * n * (k_eff + 1) + 8.0 * n * (k_eff + 1) + 8.0 * n)   # a8
+    # a8: t -= V s reads V, t and writes t; the read of V for s = V^T t is shared with the residual pass on steps without
+    # a restart (fused kernel), and is a pass of its own on restart steps and on a second Gram-Schmidt pass
+    b += reorth * (8.0 * n * (k_eff + 1) + 8.0 * n) + (reorth - (0 if restart else 1)) * 8.0 * n * (k_eff + 1)
     b += 16.0 * n                               # a9
     return b
 
@@ -176,7 +179,7 @@ def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
         if it >= 3 and kk < k_max:
             ke = kk
             for nm, b, ms in (("vtw", 8.0 * n * (kk + 1), tm[2]), ("residual", 8.0 * n * 2 * kk + 16.0 * n, tm[4]),
-                              ("orthogonalise", 2 * 8.0 * n * (ke + 1) + 8.0 * n, tm[6]), ("append", 16.0 * n, tm[7])):
+                              ("orthogonalise", 8.0 * n * (ke + 1) + 8.0 * n, tm[6]), ("append", 16.0 * n, tm[7])):
                 acc[nm][0] += b; acc[nm][1] += ms
             t_apply.append(tm[0] + tm[1])
         if conv:
