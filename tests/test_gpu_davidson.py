@@ -258,3 +258,24 @@ def test_small_eig_fast_path_equals_jacobi_fallback():
     assert fast.shape == jac.shape and len(fast) >= 20
     assert np.max(np.abs(fast[:, 0] - jac[:, 0])) <= 1e-10
     assert np.max(np.abs(fast[:, 1] - jac[:, 1]) / (1e-12 + np.abs(jac[:, 1]))) <= 1e-5
+
+
+def test_davidson_steps_are_bitwise_reproducible(lib):
+    """Fixed-order reductions everywhere (no FP atomics, readings A22/A23): two runs of the same 30 steps give identical
+    bits for lambda, ||r|| and the basis; the unit-trace diagnostic is empty unless DMRG_TRACE was set at plan creation."""
+    import torch
+    p = SMALL["cfg2_m160"]()
+    outs = []
+    for _ in range(2):
+        plan = lib.Plan(p, k_max=12, tol=1e-12)
+        V, W = plan.new_basis()
+        plan.davidson_init(V, W, start_at_argmin_diag=True)
+        k, hist = 1, []
+        for it in range(30):
+            k, lam, rho, conv = plan.davidson_step(V, W, k)
+            hist.append((lam, rho))
+        outs.append((np.array(hist), V.cpu().numpy().copy()))
+        assert len(plan.unit_trace()) == 0
+        plan.close()
+    assert np.array_equal(outs[0][0].view(np.int64), outs[1][0].view(np.int64))
+    assert np.array_equal(outs[0][1].view(np.int64), outs[1][1].view(np.int64))
