@@ -602,7 +602,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     s.workspace_bytes = 8 * (tws_elems + part_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
     s.device_bytes = p->device_bytes;
     s.kernel_launches_per_apply = 1;
-    s.kernel_launches_per_step = s.kernel_launches_per_apply + 4 + 2 * p->opt.reorth;   // +2 on a restart step
+    // apply, V^T w, small eig, residual (+ V^T t fused), { V^T t from the second pass on }, t -= V s, append; +3 on a restart step
+    s.kernel_launches_per_step = s.kernel_launches_per_apply + 3 + 2 * p->opt.reorth;
     *out = p;
     return DMRG_OK;
 }
