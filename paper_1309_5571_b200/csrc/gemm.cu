@@ -181,7 +181,11 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     if (tid == 0) s_ticket = atomicAdd(&ctrl[CTRL_TICKET], 1);
     __syncthreads();
     const int ticket = s_ticket;
-    const GemmUnit u = units[ticket];
+    // the unit descriptor lives in shared memory (read on demand) rather than in ~20 registers across the main loop
+    __shared__ GemmUnit s_u;
+    if (tid < (int)(sizeof(GemmUnit) / 4)) reinterpret_cast<int *>(&s_u)[tid] = reinterpret_cast<const int *>(units + ticket)[tid];
+    __syncthreads();
+    const GemmUnit &u = s_u;
     unsigned long long t_start = 0, t_main = 0;
     if (trace && tid == 0) t_start = globaltimer();
 
