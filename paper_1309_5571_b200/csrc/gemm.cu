@@ -80,7 +80,7 @@ struct Producer {
     bool pv, qv;
 };
 
-__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, const BasePtrs &bases, bool xvec,
+__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, bool xvec,
                                            int m0, int n0, int k0, int tid, const int *ctrl) {
     const int dep = it->dep;
     if (dep >= 0) {            // operand is a T block of this launch: wait until all its tiles are written
@@ -89,7 +89,7 @@ __device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, con
         while (ld_acquire(c) < need) __nanosleep(64);
     }
     const int pb = it->p_base, qb = it->q_base;
-    pr.P0 = bases.p[pb] + it->p_off; pr.Q0 = bases.p[qb] + it->q_off;
+    pr.P0 = bases[pb] + it->p_off; pr.Q0 = bases[qb] + it->q_off;
     pr.K = it->K; pr.k0 = k0;
     pr.pv = it->p_vec2 && (pb != BASE_X || xvec);
     pr.qv = it->q_vec2 && (qb != BASE_X || xvec);
@@ -183,7 +183,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     const int ticket = s_ticket;
     // the unit descriptor lives in shared memory (read on demand) rather than in ~20 registers across the main loop
     __shared__ GemmUnit s_u;
+    __shared__ double *s_base[BASE_COUNT];      // dynamically indexed: shared memory, not a local-memory copy of the parameter
     if (tid < (int)(sizeof(GemmUnit) / 4)) reinterpret_cast<int *>(&s_u)[tid] = reinterpret_cast<const int *>(units + ticket)[tid];
+    if (tid == 32) { s_base[BASE_X] = bases.p[BASE_X]; s_base[BASE_Y] = bases.p[BASE_Y]; s_base[BASE_T] = bases.p[BASE_T]; s_base[BASE_POOL] = bases.p[BASE_POOL]; s_base[BASE_PART] = bases.p[BASE_PART]; }
     __syncthreads();
     const GemmUnit &u = s_u;
     unsigned long long t_start = 0, t_main = 0;
@@ -212,13 +214,13 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     int p_item = u.item0, p_k0 = u.k00;      // resolved by the planner
     const int KT = u.kt_count;
     Producer pr{};
-    if (KT > 0) begin_item(pr, uitems + p_item, bases, xvec != 0, u.m0, u.n0, p_k0, tid, ctrl);
+    if (KT > 0) begin_item(pr, uitems + p_item, s_base, xvec != 0, u.m0, u.n0, p_k0, tid, ctrl);
     int c_item = p_item, c_k0 = p_k0, c_K = pr.K;
     auto produce = [&](int stage) {
         produce_tile(pr, sPbase + stage * P_STAGE, sQbase + stage * Q_STAGE, tid, rowmask16, rowmask8, colb16, colb8);
         if (pr.k0 >= pr.K) {
             p_item++;
-            if (p_item < u.item_count) begin_item(pr, uitems + p_item, bases, xvec != 0, u.m0, u.n0, 0, tid, ctrl);
+            if (p_item < u.item_count) begin_item(pr, uitems + p_item, s_base, xvec != 0, u.m0, u.n0, 0, tid, ctrl);
         }
     };
     // sub-tiles of this warp that hold real rows / columns (8-granular): padding issues no DMMA
@@ -292,7 +294,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         // split K: park the partial tile (fragment order: [slice][register pair][thread], coalesced 16-byte
         // stores); the last unit of the tile to arrive sums all slices IN SLICE ORDER (bitwise independent of
         // who is last, A22/A23) with the same thread <-> fragment mapping and writes C from registers.
-        double2 *part = reinterpret_cast<double2 *>(bases.p[BASE_PART] + u.part_off);
+        double2 *part = reinterpret_cast<double2 *>(s_base[BASE_PART] + u.part_off);
         double2 *mine = part + (long long)u.split_idx * (BM * BN / 2);
 #pragma unroll
         for (int i = 0; i < 4; i++)
@@ -331,7 +333,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         }
     }
     if (writes_c) {
-        double *C = bases.p[u.c_base] + u.c_off;
+        double *C = s_base[u.c_base] + u.c_off;
         const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
 #pragma unroll
         for (int i = 0; i < 4; i++) {
