@@ -132,6 +132,24 @@ def oracle_iteration_timer(problem, k_max: int, steps: int, warmup: int):
     return sum(flops) / sum(times) / 1e9, sum(times) / len(times) * 1e3, cores, lay.n
 
 
+def host_description() -> dict:
+    """CPU model, core count and BLAS library behind numpy (printed beside the oracle timing)."""
+    out = {"os_cpu_count": os.cpu_count()}
+    try:
+        for l in open("/proc/cpuinfo"):
+            if l.startswith("model name"):
+                out["cpu_model"] = l.split(":", 1)[1].strip()
+                break
+    except Exception:
+        pass
+    try:
+        from threadpoolctl import threadpool_info
+        out["blas"] = [{k: d.get(k) for k in ("internal_api", "version", "num_threads", "threading_layer")} for d in threadpool_info()]
+    except Exception:
+        pass
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -377,6 +395,14 @@ def run_ours(args):
         gfl, oms, cores, _ = oracle_iteration_timer(problem, k_max, osteps, 2)
         cpu_baseline = {"value": gfl, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": oms,
                         "sample": f"{osteps} consecutive O-DAV iterations of {args.config} (k = 3..{2 + osteps}) from start e_argmin(D), numpy/BLAS threads = {cores}"}
+        cpu_baseline.update(host_description())
+        try:      # the same oracle on ONE thread (the paper's CPU reference is a few-thread MKL run): 6 iterations
+            from threadpoolctl import threadpool_limits
+            with threadpool_limits(limits=1):
+                g1, ms1, _, _ = oracle_iteration_timer(problem, k_max, 6, 1)
+            cpu_baseline["one_thread"] = {"value": g1, "unit": UNIT, "ms_per_step": ms1, "sample": "6 consecutive O-DAV iterations, BLAS threads = 1"}
+        except Exception as e:
+            cpu_baseline["one_thread"] = {"error": repr(e)}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
