@@ -388,6 +388,14 @@ def run_ours(args):
         except Exception as e:   # the headline numbers above do not depend on this extra config
             dav_large = {"error": repr(e)}
 
+    curve = None
+    if world == 1:
+        try:
+            names = ["cfg2", "cfg4", "cfg5a", "heis4096"] + ([] if args.no_large else ["heis8192"])
+            curve = hpsi_curve(lib, f"cuda:{local}", max(dmma_peak, dfma_peak), names)
+        except Exception as e:
+            curve = {"error": repr(e)}
+
     # ---- oracle timed beside it (rank 0, N = 1 only): bounded sample
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
@@ -420,11 +428,47 @@ def run_ours(args):
                          "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
                          "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
                          "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
-            "davidson_hbm": dav_large,
+            "davidson_hbm": dav_large, "hpsi_curve": curve,
             "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def hpsi_curve(lib, device, fp64_peak, names):
+    """dmrg_apply_H alone at the other configs and the Heisenberg 4096 / 8192 sweep (the headline curve,
+    PAPER.md Fig. 19-20 plots the same quantity against m): time per apply, TFLOP/s on the algorithmic FLOP count (A24)
+    and fraction of the measured FP64 peak.  Seeded N(0,1) input (seed 3000+c), back to back on one stream."""
+    import torch
+    from dmrg_inputs import make_config, CONFIGS, random_vector, vector_seed
+    out = {}
+    stream = torch.cuda.current_stream()
+    for name in names:
+        problem = make_config(name)
+        plan = lib.Plan(problem, k_max=CONFIGS[name]["k_max"], device=device)
+        st = plan.stats()
+        n = plan.n
+        x = torch.from_numpy(random_vector(n, vector_seed(name, "hpsi"))).to(device)
+        y = torch.empty_like(x)
+        reps = 20 if st["flop_per_apply"] < 1e11 else 5
+        for _ in range(3):
+            plan.apply_H(x, y)
+        best = None
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                plan.apply_H(x, y)
+            e1.record(stream); torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) / reps
+            best = t if best is None else min(best, t)
+        tf = st["flop_per_apply"] / (best * 1e-3) / 1e12
+        out[name] = {"n": int(n), "flop_per_apply": int(st["flop_per_apply"]), "us_per_apply": best * 1e3, "tflops": tf,
+                     "frac_fp64_peak": tf / fp64_peak, "units": int(st["stage1_units"] + st["stage2_units"])}
+        plan.close()
+        del x, y, plan, problem
+        torch.cuda.empty_cache()
+    return out
 
 
 def main():

@@ -95,21 +95,17 @@ def test_apply_matches_oracle_full_config(lib, name):
     plan.close()
 
 
-@pytest.mark.slow
-def test_apply_matches_oracle_cfg5b_sampled(lib):
-    """Paper-scale config 5b (per-side 16384, n ~ 1.5e7): whole-vector parity is too slow for the oracle's
-    Python record loop only in memory terms, so compare on the output segments of sampled pairs, each computed
-    one by one from its own records (Eq. 11)."""
-    import torch
-    p = full_config("cfg5b")
+def _sampled_output_parity(lib, name, picks):
+    """Output segments of sampled pairs, each computed one by one from its own records (Eq. 11)."""
+    p = full_config(name)
     lay = rec.Layout(p)
     plan = lib.Plan(p, k_max=2)
-    x = random_vector(lay.n, vector_seed("cfg5b", "hpsi"))
+    x = random_vector(lay.n, vector_seed(name, "hpsi"))
     y = plan.apply_H(to_dev(x)).cpu().numpy()
     recs = rec.records(p, lay)
     sizes = np.array([int(lay.dl[i]) * int(lay.dr[k]) for i, k in lay.pairs])
-    order = np.argsort(-sizes)
-    sample = [lay.pairs[order[0]], lay.pairs[order[7]], lay.pairs[order[40]], lay.pairs[order[-1]]]
+    order = np.argsort(-sizes, kind="stable")
+    sample = [lay.pairs[order[q]] for q in picks]
     scale = np.max(np.abs(y))
     for out in sample:
         acc = np.zeros((int(lay.dl[out[0]]), int(lay.dr[out[1]])))
@@ -121,10 +117,27 @@ def test_apply_matches_oracle_cfg5b_sampled(lib):
             T = T if B is None else T @ B.T
             acc += c * T
         got = lay.seg(y, *out)
-        assert np.max(np.abs(got - acc)) <= HPSI_RTOL * scale
+        assert np.max(np.abs(got - acc)) <= HPSI_RTOL * scale, (name, out)
     st = plan.stats()
-    assert st["device_bytes"] < 40e9
     plan.close()
+    return st
+
+
+@pytest.mark.slow
+def test_apply_matches_oracle_cfg5b_sampled(lib):
+    """Paper-scale config 5b (per-side 16384, n ~ 1.5e7): whole-vector parity is too slow for the oracle's
+    Python record loop only in memory terms, so compare on the output segments of sampled pairs: the largest,
+    two from the middle of the size order and the smallest."""
+    st = _sampled_output_parity(lib, "cfg5b", [0, 7, 40, -1])
+    assert st["device_bytes"] < 40e9
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,picks", [("heis4096", [0, 1, 5, 12, -1]), ("heis8192", [0, 3, 9, -1])])
+def test_apply_matches_oracle_sweep_sampled(lib, name, picks):
+    """The Heisenberg 4096 / 8192 points of the headline curve (8192 is the paper's m = 4096 shape,
+    Table 5) in the launch configuration bench.py `hpsi_curve` times."""
+    _sampled_output_parity(lib, name, picks)
 
 
 def test_unaligned_vectors_and_bitwise_determinism(lib):
