@@ -146,7 +146,7 @@ const char *dmrg_last_error(dmrg_handle_t h);
 
 /* y = H_SB x on the target sector: Eq. 11 over all records (Alg. 3 line 2).
  * x, y DEVICE, n doubles each, must not overlap; y is overwritten.  Asynchronous on the
- * stream; no allocation; two kernel launches. */
+ * stream; no allocation; one kernel launch (both GEMM stages of every record). */
 int dmrg_apply_H(dmrg_handle_t h, const double *x, double *y, void *cuda_stream);
 
 /* Starts a Davidson run (Alg. 3 "Require"): V(:,0) = x0/||x0||, k = 1,
@@ -165,9 +165,20 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
  * In: *k = number of orthonormal columns held in V (W(:,0..k-2) = H V(:,0..k-2), B as
  * left by the previous call).  Out: *k updated (k+1, or 2 after a restart; unchanged when
  * converged), *lambda, *resnorm, *converged (HOST).  Synchronises the stream once to read
- * these three numbers.  Returns DMRG_E_NUMERIC on breakdown (A18/step 9). */
+ * these three numbers.  Returns DMRG_E_NUMERIC on breakdown (A18/step 9).
+ * With lambda, resnorm and converged ALL NULL the step is only enqueued (no synchronisation,
+ * the way dmrg_lowest_eigenpair runs its loop): *k is advanced as if the step did not
+ * converge (the basis size is a host-known function of the step count), the convergence
+ * test still runs on the device and every step enqueued after it fires is a no-op that
+ * leaves V, W, B and the reported state untouched; read the state with dmrg_davidson_poll. */
 int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k,
                        double *lambda, double *resnorm, int32_t *converged, void *cuda_stream);
+
+/* Synchronises the stream and reports the state after the last EXECUTED (not no-op) step:
+ * lambda, rho = ||r|| (Alg. 3 lines 4-7), converged flag, number of executed iterations
+ * since dmrg_davidson_init (HOST; any may be NULL).  DMRG_E_NUMERIC on breakdown. */
+int dmrg_davidson_poll(dmrg_handle_t h, double *lambda, double *resnorm, int32_t *converged,
+                       int32_t *iters, void *cuda_stream);
 
 /* Small-matrix state of the last step for lock-step tests: B (k_max x k_max, row-major)
  * and y (k_max) copied to HOST arrays (either may be NULL).  dmrg_set_small loads B

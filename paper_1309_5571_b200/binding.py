@@ -21,7 +21,7 @@ DMRG_HEISENBERG, DMRG_HUBBARD = 1, 2
 
 EXPORTS = [
     "dmrg_plan_create", "dmrg_plan_destroy", "dmrg_get_layout", "dmrg_get_stats", "dmrg_get_diag",
-    "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_get_small",
+    "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_davidson_poll", "dmrg_get_small",
     "dmrg_set_small", "dmrg_ritz_vector", "dmrg_lowest_eigenpair", "dmrg_gemv_trans", "dmrg_gemv_sub",
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
 ]
@@ -92,6 +92,7 @@ def load_library():
         "dmrg_apply_H": [vp, vp, vp, vp],
         "dmrg_davidson_init": [vp, vp, i32, vp, vp, i64, vp],
         "dmrg_davidson_step": [vp, vp, vp, i64, pi32, pdbl, pdbl, pi32, vp],
+        "dmrg_davidson_poll": [vp, pdbl, pdbl, pi32, pi32, vp],
         "dmrg_get_small": [vp, pdbl, pdbl, vp],
         "dmrg_set_small": [vp, pdbl, vp],
         "dmrg_ritz_vector": [vp, vp, i64, i32, vp, vp],
@@ -242,6 +243,21 @@ class Plan:
         ldv = V.stride(0) if V.dim() == 2 else self.n
         self._check(self._lib.dmrg_davidson_init(self._h, _ptr(x0), int(bool(start_at_argmin_diag)), _ptr(V), _ptr(W),
                                                  int(ldv), _stream_ptr(stream)))
+
+    def davidson_enqueue(self, V, W, k: int, stream=None) -> int:
+        """dmrg_davidson_step with NULL outputs: enqueue only, returns the next basis size; see davidson_poll."""
+        kk = C.c_int32(int(k))
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_davidson_step(self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), None, None, None,
+                                                 _stream_ptr(stream)))
+        return int(kk.value)
+
+    def davidson_poll(self, stream=None) -> Tuple[float, float, bool, int]:
+        """(lambda, rho, converged, executed iterations) after a stream synchronisation."""
+        lam, rho, conv, it = C.c_double(), C.c_double(), C.c_int32(), C.c_int32()
+        self._check(self._lib.dmrg_davidson_poll(self._h, C.byref(lam), C.byref(rho), C.byref(conv), C.byref(it),
+                                                 _stream_ptr(stream)))
+        return float(lam.value), float(rho.value), bool(conv.value), int(it.value)
 
     def davidson_step(self, V, W, k: int, stream=None) -> Tuple[int, float, float, bool]:
         kk, lam, rho, conv = C.c_int32(int(k)), C.c_double(), C.c_double(), C.c_int32()

@@ -107,6 +107,10 @@ int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32
     int k_next = *k;
     int rc = dav_enqueue_step(p, V, W, ldv, *k, S(stream), &k_next);
     if (rc != DMRG_OK) return rc;
+    if (!lambda && !resnorm && !converged) {   // enqueue only: no stream synchronisation (see dmrg_davidson_poll)
+        *k = k_next;
+        return DMRG_OK;
+    }
     rc = read_state(p, S(stream), false);
     if (rc != DMRG_OK) return rc;
     const DavState &st = *p->state_host;
@@ -122,6 +126,21 @@ int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32
             p->timing.ms[q] = ms;
         }
     }
+    return DMRG_OK;
+}
+
+int dmrg_davidson_poll(dmrg_handle_t h, double *lambda, double *resnorm, int32_t *converged, int32_t *iters,
+                       void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    int rc = read_state(p, S(stream), false);
+    if (rc != DMRG_OK) return rc;
+    const DavState &st = *p->state_host;
+    if (lambda) *lambda = st.lambda;
+    if (resnorm) *resnorm = st.rho;
+    if (converged) *converged = (st.done == 1) ? 1 : 0;
+    if (iters) *iters = st.iters;
+    if (st.error || st.done == 2) return fail(p, DMRG_E_NUMERIC, "Davidson breakdown: zero or non-finite norm");
     return DMRG_OK;
 }
 

@@ -279,3 +279,42 @@ def test_davidson_steps_are_bitwise_reproducible(lib):
         plan.close()
     assert np.array_equal(outs[0][0].view(np.int64), outs[1][0].view(np.int64))
     assert np.array_equal(outs[0][1].view(np.int64), outs[1][1].view(np.int64))
+
+
+def test_enqueued_steps_equal_synchronous_steps(lib):
+    """dmrg_davidson_step with NULL outputs only enqueues (include/dmrg_b200.h); 30 enqueued steps + one
+    dmrg_davidson_poll must leave exactly the state of 30 synchronising calls (bitwise: same kernels, same order),
+    and steps enqueued after the device-side convergence test fired must be no-ops."""
+    import torch
+    p = SMALL["heis_syn_m300_ragged"]()
+    plan = lib.Plan(p, k_max=12, tol=1e-9)
+    Va, Wa = plan.new_basis()
+    Vb, Wb = plan.new_basis()
+    plan.davidson_init(Va, Wa, start_at_argmin_diag=True)
+    k, ks = 1, []
+    for _ in range(30):
+        k, lam_a, rho_a, conv = plan.davidson_step(Va, Wa, k)
+        ks.append(k)
+        assert not conv
+    plan.davidson_init(Vb, Wb, start_at_argmin_diag=True)
+    k = 1
+    for i in range(30):
+        k = plan.davidson_enqueue(Vb, Wb, k)
+        assert k == ks[i]
+    lam_b, rho_b, conv_b, iters_b = plan.davidson_poll()
+    assert (lam_b, rho_b, conv_b, iters_b) == (lam_a, rho_a, False, 30)
+    assert torch.equal(Va, Vb) and torch.equal(Wa, Wb)
+    # run on to convergence, then enqueue 5 more: state, V and W must not move
+    for _ in range(2000):
+        k, lam, rho, conv = plan.davidson_step(Vb, Wb, k)
+        if conv:
+            break
+    assert conv
+    lam0, rho0, c0, it0 = plan.davidson_poll()
+    Vc, Wc = Vb.clone(), Wb.clone()
+    kk = k
+    for _ in range(5):
+        kk = plan.davidson_enqueue(Vb, Wb, kk)
+    assert plan.davidson_poll() == (lam0, rho0, True, it0)
+    assert torch.equal(Vb, Vc) and torch.equal(Wb, Wc)
+    plan.close()
