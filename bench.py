@@ -15,9 +15,11 @@ the C ABI (dmrg_davidson_step), basis size cycling 1..k_max as in a real run.
 
 value   = algorithmic FP64 GFLOP/s of the whole step (A24 FLOP of the apply + BLAS-2 FLOP) with
           everything resident in HBM; L2 is flushed between timed steps (outside the event pairs).
-e2e     = same metric with host buffers: every step copies the newest basis vector host->device from
-          pinned memory and the projected vector W(:,k) device->host (the per-iteration crossing of the
-          paper's hybrid scheme: H2D of the input, D2H of the output, Alg. 7).
+e2e     = same metric with host buffers through dmrg_davidson_step_host: every step copies the newest basis
+          vector host->device from pinned memory and the projected vector W(:,k) device->host (the
+          per-iteration crossing of the paper's hybrid scheme: H2D of the input, D2H of the output,
+          PAPER.md:L263, L432-445 Alg. 7); the D2H runs on a side stream under lines 3-13, one
+          synchronising call per step.
 roofline= the grouped DMMA kernel (one launch per step) against the FP64 DMMA peak measured live.
 davidson_hbm = the BLAS-2 kernels timed inside running steps at config 5b (n ~ 1.5e7: V, W >> L2) against the
           measured HBM copy bandwidth (the >= 75 % judgement is taken where V >> L2).
@@ -280,16 +282,12 @@ def run_ours(args):
             if j >= 0:
                 ev[j][0].record(stream)
                 ks.append(k)
-            if host_io:   # newest basis vector in, projected vector out (pinned host buffers)
-                V[k - 1, :n].copy_(hx, non_blocking=True)
-            k_prev = k
-            if enqueue_only:
+            if host_io:   # newest basis vector in, projected vector out (pinned host buffers): dmrg_davidson_step_host
+                k, lam, rho, conv = plan.davidson_step_host(V, W, k, hx, hw)     # copies + step, synchronises
+            elif enqueue_only:
                 k, conv = plan.davidson_enqueue(V, W, k), False
             else:
                 k, lam, rho, conv = plan.davidson_step(V, W, k)
-            if host_io:
-                hw.copy_(W[k_prev - 1, :n], non_blocking=True)
-                stream.synchronize()
             if j >= 0:
                 ev[j][1].record(stream)
             if enqueue_only and ((it + 1) % 8 == 0 or it + 1 == warmup + steps):

@@ -174,6 +174,20 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
 int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k,
                        double *lambda, double *resnorm, int32_t *converged, void *cuda_stream);
 
+/* dmrg_davidson_step for a caller that keeps (part of) the basis on the HOST -- the setting of the
+ * paper's hybrid code, where each new basis vector is uploaded and H_SB x downloaded every
+ * iteration (Alg. 7 lines 3 and 7, L432-445).  v_in_host (n doubles, or NULL) is copied into
+ * V(:,k-1) on the stream before line 2; w_out_host (n doubles, or NULL) receives W(:,k-1) =
+ * H_SB V(:,k-1), copied on a plan-owned side stream as soon as the projection has finished so
+ * that the transfer overlaps lines 3-13 (on a restart step the collapse waits for it).  Pinned
+ * host memory is needed for the copies to be asynchronous.  Always synchronises (stream and
+ * side stream) before returning; the other arguments and the return value are those of
+ * dmrg_davidson_step.  If the run had already converged the step is a no-op and w_out_host
+ * receives W(:,k-1) as it stands. */
+int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k,
+                            const double *v_in_host, double *w_out_host, double *lambda,
+                            double *resnorm, int32_t *converged, void *cuda_stream);
+
 /* Synchronises the stream and reports the state after the last EXECUTED (not no-op) step:
  * lambda, rho = ||r|| (Alg. 3 lines 4-7), converged flag, number of executed iterations
  * since dmrg_davidson_init (HOST; any may be NULL).  DMRG_E_NUMERIC on breakdown. */

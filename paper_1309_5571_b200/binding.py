@@ -21,7 +21,7 @@ DMRG_HEISENBERG, DMRG_HUBBARD = 1, 2
 
 EXPORTS = [
     "dmrg_plan_create", "dmrg_plan_destroy", "dmrg_get_layout", "dmrg_get_stats", "dmrg_get_diag",
-    "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_davidson_poll", "dmrg_get_small",
+    "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_davidson_step_host", "dmrg_davidson_poll", "dmrg_get_small",
     "dmrg_set_small", "dmrg_ritz_vector", "dmrg_lowest_eigenpair", "dmrg_gemv_trans", "dmrg_gemv_sub",
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
 ]
@@ -92,6 +92,7 @@ def load_library():
         "dmrg_apply_H": [vp, vp, vp, vp],
         "dmrg_davidson_init": [vp, vp, i32, vp, vp, i64, vp],
         "dmrg_davidson_step": [vp, vp, vp, i64, pi32, pdbl, pdbl, pi32, vp],
+        "dmrg_davidson_step_host": [vp, vp, vp, i64, pi32, vp, vp, pdbl, pdbl, pi32, vp],
         "dmrg_davidson_poll": [vp, pdbl, pdbl, pi32, pi32, vp],
         "dmrg_get_small": [vp, pdbl, pdbl, vp],
         "dmrg_set_small": [vp, pdbl, vp],
@@ -258,6 +259,18 @@ class Plan:
         self._check(self._lib.dmrg_davidson_poll(self._h, C.byref(lam), C.byref(rho), C.byref(conv), C.byref(it),
                                                  _stream_ptr(stream)))
         return float(lam.value), float(rho.value), bool(conv.value), int(it.value)
+
+    def davidson_step_host(self, V, W, k: int, v_in_host=None, w_out_host=None, stream=None) -> Tuple[int, float, float, bool]:
+        """dmrg_davidson_step_host: v_in_host / w_out_host are CPU float64 tensors of n elements (pinned for overlap)."""
+        for nm, t in (("v_in_host", v_in_host), ("w_out_host", w_out_host)):
+            if t is not None and (t.is_cuda or t.dtype != _torch().float64 or t.numel() != self.n or not t.is_contiguous()):
+                raise ValueError(f"{nm} must be a contiguous CPU float64 tensor of {self.n} elements")
+        kk, lam, rho, conv = C.c_int32(int(k)), C.c_double(), C.c_double(), C.c_int32()
+        ldv = V.stride(0) if V.dim() == 2 else self.n
+        self._check(self._lib.dmrg_davidson_step_host(
+            self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), _ptr(v_in_host), _ptr(w_out_host),
+            C.byref(lam), C.byref(rho), C.byref(conv), _stream_ptr(stream)))
+        return int(kk.value), float(lam.value), float(rho.value), bool(conv.value)
 
     def davidson_step(self, V, W, k: int, stream=None) -> Tuple[int, float, float, bool]:
         kk, lam, rho, conv = C.c_int32(int(k)), C.c_double(), C.c_double(), C.c_int32()

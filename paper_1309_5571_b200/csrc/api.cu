@@ -98,27 +98,24 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
     return dav_init(p, x0, start_at_argmin_diag, V, W, ldv, S(stream));
 }
 
-int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, double *lambda,
-                       double *resnorm, int32_t *converged, void *stream) {
-    if (!h) return DMRG_E_INVALID_ARG;
-    Plan *p = P(h);
-    if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step: NULL argument");
+static int step_common(Plan *p, double *V, double *W, int64_t ldv, int32_t *k, double *lambda, double *resnorm,
+                       int32_t *converged, cudaStream_t st, bool enqueue_only) {
     if (p->timing.enabled) ensure_timing(p);
     int k_next = *k;
-    int rc = dav_enqueue_step(p, V, W, ldv, *k, S(stream), &k_next);
+    int rc = dav_enqueue_step(p, V, W, ldv, *k, st, &k_next);
     if (rc != DMRG_OK) return rc;
-    if (!lambda && !resnorm && !converged) {   // enqueue only: no stream synchronisation (see dmrg_davidson_poll)
+    if (enqueue_only) {   // no stream synchronisation (see dmrg_davidson_poll)
         *k = k_next;
         return DMRG_OK;
     }
-    rc = read_state(p, S(stream), false);
+    rc = read_state(p, st, false);
     if (rc != DMRG_OK) return rc;
-    const DavState &st = *p->state_host;
-    if (lambda) *lambda = st.lambda;
-    if (resnorm) *resnorm = st.rho;
-    if (converged) *converged = (st.done == 1) ? 1 : 0;
-    if (st.error || st.done == 2) return fail(p, DMRG_E_NUMERIC, "Davidson breakdown: zero or non-finite norm");
-    if (st.done != 1) *k = k_next;
+    const DavState &s = *p->state_host;
+    if (lambda) *lambda = s.lambda;
+    if (resnorm) *resnorm = s.rho;
+    if (converged) *converged = (s.done == 1) ? 1 : 0;
+    if (s.error || s.done == 2) return fail(p, DMRG_E_NUMERIC, "Davidson breakdown: zero or non-finite norm");
+    if (s.done != 1) *k = k_next;
     if (p->timing.enabled) {
         for (int q = 0; q < 8; q++) {
             float ms = 0.f;
@@ -127,6 +124,39 @@ int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32
         }
     }
     return DMRG_OK;
+}
+
+int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, double *lambda,
+                       double *resnorm, int32_t *converged, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step: NULL argument");
+    return step_common(p, V, W, ldv, k, lambda, resnorm, converged, S(stream), !lambda && !resnorm && !converged);
+}
+
+int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, const double *v_in_host,
+                            double *w_out_host, double *lambda, double *resnorm, int32_t *converged, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_host: NULL argument");
+    if (*k < 1 || *k > p->opt.k_max || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_host: k or ldv out of range");
+    cudaStream_t st = S(stream);
+    if (w_out_host && !p->side) {
+        cudaError_t e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_apply, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
+        if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    }
+    if (v_in_host)
+        cudaMemcpyAsync(V + (long long)(*k - 1) * ldv, v_in_host, sizeof(double) * p->n, cudaMemcpyHostToDevice, st);
+    p->w_out_host = w_out_host;
+    int rc = step_common(p, V, W, ldv, k, lambda, resnorm, converged, st, false);
+    p->w_out_host = nullptr;
+    if (w_out_host) {
+        cudaError_t e = cudaStreamSynchronize(p->side);
+        if (rc == DMRG_OK && e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    }
+    return rc;
 }
 
 int dmrg_davidson_poll(dmrg_handle_t h, double *lambda, double *resnorm, int32_t *converged, int32_t *iters,

@@ -117,6 +117,10 @@ struct Plan {
     std::string err;
     Timing timing;
     int sm_count = 148;
+    // dmrg_davidson_step_host: W(:,k-1) leaves on a side stream as soon as the projection is done
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_apply = nullptr, ev_side = nullptr;
+    double *w_out_host = nullptr;       // non-null only while such a step is being enqueued
 };
 
 void set_global_error(const std::string &s);

@@ -616,6 +616,9 @@ void plan_free(Plan *p) {
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
     cudaFree(p->Vown); cudaFree(p->Wown);
     if (p->timing.created) for (auto &e : p->timing.ev) cudaEventDestroy(e);
+    if (p->ev_apply) cudaEventDestroy(p->ev_apply);
+    if (p->ev_side) cudaEventDestroy(p->ev_side);
+    if (p->side) cudaStreamDestroy(p->side);
     delete p;
 }
 

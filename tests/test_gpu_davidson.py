@@ -318,3 +318,48 @@ def test_enqueued_steps_equal_synchronous_steps(lib):
     assert plan.davidson_poll() == (lam0, rho0, True, it0)
     assert torch.equal(Vb, Vc) and torch.equal(Wb, Wc)
     plan.close()
+
+
+def test_step_host_equals_step_with_manual_copies(lib):
+    """dmrg_davidson_step_host (H2D of V(:,k-1) before line 2, D2H of W(:,k-1) on a side stream overlapping lines
+    3-13) must give bitwise the results of dmrg_davidson_step + the two copies done by hand, across restart steps
+    (k == k_max, where the collapse rewrites W) and with either host pointer NULL."""
+    import torch
+    p = SMALL["heis_syn_m300_ragged"]()
+    plan = lib.Plan(p, k_max=4, tol=1e-12)
+    n = plan.n
+    Va, Wa = plan.new_basis()
+    Vb, Wb = plan.new_basis()
+    hx = torch.empty(n, dtype=torch.float64).pin_memory()
+    hw = torch.empty(n, dtype=torch.float64).pin_memory()
+    plan.davidson_init(Va, Wa, start_at_argmin_diag=True)
+    ref = []
+    k = 1
+    for _ in range(14):
+        kp = k
+        k, lam, rho, conv = plan.davidson_step(Va, Wa, k)
+        ref.append((k, lam, rho, conv, Va[k - 1, :n].cpu().clone()))
+        assert not conv
+    # W(:,kp-1) right after the projection is not observable after a restart step, so recompute it for the check
+    plan.davidson_init(Vb, Wb, start_at_argmin_diag=True)
+    k = 1
+    hx.copy_(Vb[0, :n])
+    for i in range(14):
+        kp = k
+        x_dev = Vb[kp - 1, :n].clone()
+        Vb[kp - 1, :n].zero_()                       # the step must take its input from the host buffer
+        use_in = hx if i % 5 != 4 else None
+        if use_in is None:
+            Vb[kp - 1, :n].copy_(x_dev)
+        use_out = hw if i % 7 != 6 else None
+        hw.fill_(float("nan"))
+        k, lam, rho, conv = plan.davidson_step_host(Vb, Wb, k, use_in, use_out)
+        assert (k, lam, rho, conv) == ref[i][:4]
+        if use_out is not None:
+            assert torch.equal(hw, plan.apply_H(x_dev).cpu())
+        assert torch.equal(Vb[k - 1, :n].cpu(), ref[i][4])
+        hx.copy_(Vb[k - 1, :n])
+    assert torch.equal(Va, Vb) and torch.equal(Wa, Wb)
+    with pytest.raises(ValueError):
+        plan.davidson_step_host(Vb, Wb, k, torch.empty(n - 1, dtype=torch.float64), None)
+    plan.close()
