@@ -113,7 +113,7 @@ typedef struct {
     int64_t device_bytes;      /* everything the plan allocated on the device             */
     int32_t kernel_launches_per_apply;
     int32_t kernel_launches_per_step;  /* dmrg_davidson_step at reorth passes = options   */
-    int64_t flop_stage1, flop_stage2;  /* split of flop_per_apply over the two launches    */
+    int64_t flop_stage1, flop_stage2;  /* split of flop_per_apply over the two GEMM stages */
     int64_t launches;                  /* kernels launched by the hot-path entry points of
                                           this plan since it was created (host-side count) */
 } dmrg_stats;

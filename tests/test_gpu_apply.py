@@ -229,3 +229,46 @@ def test_zero_couplings_reduce_to_sylvester_form(lib):
         X = lay.seg(x, i, k)
         assert np.max(np.abs(lay.seg(y, i, k) - (HL[i] @ X + X @ HR[k].T))) <= 1e-11
     plan.close()
+
+
+def _fuzz_problem(seed):
+    """Seeded random problem shapes beyond the named configs: per-side dimension, sector count, profile width,
+    couplings and model all drawn from the seed (generators of dmrg_inputs, no arithmetic of the method here)."""
+    from dmrg_inputs import hubbard_synthetic
+    rng = np.random.default_rng(90000 + seed)
+    m = int(rng.integers(20, 700))
+    if seed % 2 == 0:
+        qmax = int(rng.integers(1, 7))
+        return heisenberg_synthetic(m, qmax, ["gaussian", "binomial"][int(rng.integers(0, 2))], float(rng.uniform(-1.5, 1.5)),
+                                    seed=int(rng.integers(1, 1 << 30)), J=float(rng.uniform(0.2, 2.0)),
+                                    sigma=float(rng.uniform(0.6, 2.5)), sz_mode=["dense", "label"][int(rng.integers(0, 2))])
+    ell = int(rng.integers(1, 5))
+    return hubbard_synthetic(max(m, (ell + 1) ** 2), float(rng.uniform(0.0, 10.0)), seed=int(rng.integers(1, 1 << 30)),
+                             t=float(rng.uniform(0.3, 2.0)), ell=ell, sigma=float(rng.uniform(0.7, 2.0)))
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_apply_matches_oracle_fuzz(lib, seed, monkeypatch):
+    """Random shapes x two planner granularities: the default, and 200 work units per SM, which splits the K range of
+    every output tile as finely as the planner allows (split-K partials, last-arriver reduction and the stage-1 ->
+    stage-2 counters all exercised on small problems).  Same bar as everywhere: 1e-10 in the max norm, bitwise
+    reproducible, and both plans agree to rounding."""
+    import torch
+    p = _fuzz_problem(seed)
+    lay = rec.Layout(p)
+    x = random_vector(lay.n, 100 + seed)
+    want = oracle_apply(p, lay)(x)
+    xd = to_dev(x)
+    for ups in (None, "200"):
+        if ups is None:
+            monkeypatch.delenv("DMRG_UNITS_PER_SM", raising=False)
+        else:
+            monkeypatch.setenv("DMRG_UNITS_PER_SM", ups)
+        plan = lib.Plan(p, k_max=2)
+        assert plan.n == lay.n
+        y = plan.apply_H(xd)
+        y2 = plan.apply_H(xd)
+        torch.cuda.synchronize()
+        assert torch.equal(y, y2)
+        assert rel_maxnorm(y.cpu().numpy(), want) <= HPSI_RTOL, (seed, ups)
+        plan.close()
