@@ -29,6 +29,21 @@ def small_problems():
     }
 
 
+def fuzz_problem(seed, m_max=700):
+    """Seeded random problem shapes beyond the named configs: per-side dimension, sector count, profile width,
+    couplings and model all drawn from the seed (generators of dmrg_inputs, no arithmetic of the method here)."""
+    rng = np.random.default_rng(90000 + seed)
+    m = int(rng.integers(20, m_max))
+    if seed % 2 == 0:
+        qmax = int(rng.integers(1, 7))
+        return heisenberg_synthetic(m, qmax, ["gaussian", "binomial"][int(rng.integers(0, 2))], float(rng.uniform(-1.5, 1.5)),
+                                    seed=int(rng.integers(1, 1 << 30)), J=float(rng.uniform(0.2, 2.0)),
+                                    sigma=float(rng.uniform(0.6, 2.5)), sz_mode=["dense", "label"][int(rng.integers(0, 2))])
+    ell = int(rng.integers(1, 5))
+    return hubbard_synthetic(max(m, (ell + 1) ** 2), float(rng.uniform(0.0, 10.0)), seed=int(rng.integers(1, 1 << 30)),
+                             t=float(rng.uniform(0.3, 2.0)), ell=ell, sigma=float(rng.uniform(0.7, 2.0)))
+
+
 @functools.lru_cache(maxsize=4)
 def full_config(name):
     return make_config(name)

@@ -10,7 +10,7 @@ from dmrg_inputs import random_vector, heisenberg_synthetic
 from dmrg_inputs.problem import Problem, Sectors, BlockOp, HEISENBERG
 from dmrg_inputs.synthetic import vector_seed
 from oracle import blocks, rec, ed
-from gpu_common import small_problems, full_config, oracle_apply, rel_maxnorm, to_dev, HPSI_RTOL
+from gpu_common import small_problems, full_config, fuzz_problem, oracle_apply, rel_maxnorm, to_dev, HPSI_RTOL
 
 pytestmark = pytest.mark.gpu
 SMALL = small_problems()
@@ -231,22 +231,6 @@ def test_zero_couplings_reduce_to_sylvester_form(lib):
     plan.close()
 
 
-def _fuzz_problem(seed):
-    """Seeded random problem shapes beyond the named configs: per-side dimension, sector count, profile width,
-    couplings and model all drawn from the seed (generators of dmrg_inputs, no arithmetic of the method here)."""
-    from dmrg_inputs import hubbard_synthetic
-    rng = np.random.default_rng(90000 + seed)
-    m = int(rng.integers(20, 700))
-    if seed % 2 == 0:
-        qmax = int(rng.integers(1, 7))
-        return heisenberg_synthetic(m, qmax, ["gaussian", "binomial"][int(rng.integers(0, 2))], float(rng.uniform(-1.5, 1.5)),
-                                    seed=int(rng.integers(1, 1 << 30)), J=float(rng.uniform(0.2, 2.0)),
-                                    sigma=float(rng.uniform(0.6, 2.5)), sz_mode=["dense", "label"][int(rng.integers(0, 2))])
-    ell = int(rng.integers(1, 5))
-    return hubbard_synthetic(max(m, (ell + 1) ** 2), float(rng.uniform(0.0, 10.0)), seed=int(rng.integers(1, 1 << 30)),
-                             t=float(rng.uniform(0.3, 2.0)), ell=ell, sigma=float(rng.uniform(0.7, 2.0)))
-
-
 @pytest.mark.parametrize("seed", range(16))
 def test_apply_matches_oracle_fuzz(lib, seed, monkeypatch):
     """Random shapes x two planner granularities: the default, and 200 work units per SM, which splits the K range of
@@ -254,7 +238,7 @@ def test_apply_matches_oracle_fuzz(lib, seed, monkeypatch):
     stage-2 counters all exercised on small problems).  Same bar as everywhere: 1e-10 in the max norm, bitwise
     reproducible, and both plans agree to rounding."""
     import torch
-    p = _fuzz_problem(seed)
+    p = fuzz_problem(seed)
     lay = rec.Layout(p)
     x = random_vector(lay.n, 100 + seed)
     want = oracle_apply(p, lay)(x)

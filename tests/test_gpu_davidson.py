@@ -10,7 +10,7 @@ import pytest
 from dmrg_inputs import random_vector
 from dmrg_inputs.synthetic import vector_seed
 from oracle import blocks, rec, kron, davidson as odav
-from gpu_common import (small_problems, full_config, oracle_apply, to_dev, basis_to_numpy,
+from gpu_common import (small_problems, full_config, fuzz_problem, oracle_apply, to_dev, basis_to_numpy,
                         LAMBDA_ATOL, OVERLAP_DEF)
 
 pytestmark = pytest.mark.gpu
@@ -362,4 +362,39 @@ def test_step_host_equals_step_with_manual_copies(lib):
     assert torch.equal(Va, Vb) and torch.equal(Wa, Wb)
     with pytest.raises(ValueError):
         plan.davidson_step_host(Vb, Wb, k, torch.empty(n - 1, dtype=torch.float64), None)
+    plan.close()
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_trajectory_parity_fuzz(lib, seed):
+    """Random problem shapes (tests/gpu_common.fuzz_problem) x random basis limit k_max in [3, 32] and reorth in {1, 2}:
+    the GPU and the oracle run 45 iterations independently from start (D) -- through several restarts for the small
+    k_max -- and must report the same (lambda, ||r||) at every iteration; the driver then has to reach the oracle's
+    converged eigenvalue from the seeded random start (R)."""
+    rng = np.random.default_rng(500 + seed)
+    p = fuzz_problem(100 + seed, m_max=260)
+    k_max, reorth = int(rng.integers(3, 33)), int(rng.integers(1, 3))
+    lay = rec.Layout(p)
+    D = rec.diag_H(p, lay)
+    apply = oracle_apply(p, lay)
+    ores = odav.davidson_solve(apply, D, odav.start_argmin_diag(D), k_max, 1e-10, 45, reorth)
+    plan = lib.Plan(p, k_max=k_max, tol=1e-10, reorth=reorth, max_iter=4000)
+    V, W = plan.new_basis()
+    plan.davidson_init(V, W, start_at_argmin_diag=True)
+    k = 1
+    for it, (lo, ro) in enumerate(ores["history"]):
+        k, lam, rho, conv = plan.davidson_step(V, W, k)
+        assert abs(lam - lo) <= LAMBDA_ATOL, (seed, it, k_max, reorth)
+        assert abs(rho - ro) <= 1e-9 + 1e-6 * ro, (seed, it, k_max, reorth)
+        if conv:
+            break
+    x0 = random_vector(lay.n, 2000 + seed)
+    full = odav.davidson_solve(apply, D, x0, k_max, 1e-10, 4000, reorth)
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(x0=to_dev(x0))
+    if full["converged"]:
+        assert rc == 0 and abs(lam - full["lam"]) <= LAMBDA_ATOL
+        assert abs(abs(x.cpu().numpy() @ full["x"]) - 1.0) <= OVERLAP_DEF
+        # iteration counts are not unique: after a few restarts rounding-level differences change the path to
+        # the same eigenpair (the first 45 iterations above are compared one by one); only guard against a stall
+        assert full["iters"] / 1.6 - 10 <= iters <= full["iters"] * 1.6 + 10, (seed, k_max, reorth, iters, full["iters"])
     plan.close()
