@@ -66,6 +66,23 @@ def test_argument_errors_without_gpu(lib):
     assert lib.dmrg_plan_create(None, None, None) == binding.DMRG_E_INVALID_ARG
     assert lib.dmrg_apply_H(None, None, None, None) == binding.DMRG_E_INVALID_ARG
     assert lib.dmrg_plan_destroy(None) == binding.DMRG_E_INVALID_ARG
+    # every entry point that takes a handle rejects a NULL one before touching the device
+    k = C.c_int32(1)
+    assert lib.dmrg_davidson_init(None, None, 0, None, None, 0, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_davidson_step(None, None, None, 0, C.byref(k), None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_davidson_step_host(None, None, None, 0, C.byref(k), None, None, None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_davidson_poll(None, None, None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_lowest_eigenpair(None, None, 0, None, None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_ritz_vector(None, None, 0, 1, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_get_small(None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_set_small(None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_gemv_trans(None, None, 0, 1, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_gemv_sub(None, None, 0, 1, None, None, None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_get_stats(None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_get_unit_trace(None, None, 0, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_set_timing(None, 1) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_get_timing(None, None) == binding.DMRG_E_INVALID_ARG
+    assert lib.dmrg_probe_fp64_peak(5, 1, None, None) == binding.DMRG_E_INVALID_ARG
     pr = binding._Problem()
     pr.model = 7
     assert lib.dmrg_plan_create(C.byref(pr), None, C.byref(h)) == binding.DMRG_E_INVALID_ARG
