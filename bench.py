@@ -179,6 +179,42 @@ def workload_config(name, cfg, n, stats):
     return c
 
 
+def gemv_trans_probe(plan, V, W, flush, hbm_peak):
+    """The paper's own BLAS-2 benchmark shape (Fig. 6-10: V^T x for a ~5e5 x 16..20 matrix, no host
+    transfer): dmrg_gemv_trans alone on this config's n, one launch per event pair, L2 flushed before every launch
+    (cold) and back to back (warm; V fits the 126 MB L2 up to k ~ 20 at cfg3).  Context only: the >= 75 % HBM judgement
+    is taken at cfg5b (`davidson_hbm`)."""
+    import torch
+    n = plan.n
+    stream = torch.cuda.current_stream()
+    out = {"n": int(n), "paper": "114.7 GB/s (GTX 570, 75 % of 152), 143.7 GB/s (K20, 69 % of 208) at 16 x 5e5, PAPER.md:L316-326"}
+    res = torch.empty(32, dtype=torch.float64, device=V.device)
+    w = W[0, :n]
+    for k in (16, 20):
+        if k > V.shape[0]:
+            continue
+        cold = []
+        for _ in range(12):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); plan.gemv_trans(V, k, w, res); e1.record(stream)
+            torch.cuda.synchronize()
+            cold.append(e0.elapsed_time(e1))
+        for _ in range(3):
+            plan.gemv_trans(V, k, w, res)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(50):
+            plan.gemv_trans(V, k, w, res)
+        e1.record(stream); torch.cuda.synchronize()
+        warm = e0.elapsed_time(e1) / 50
+        b = 8.0 * n * (k + 1) + 8.0 * k
+        c = float(np.median(cold))
+        out[f"k{k}"] = {"us_cold": c * 1e3, "gbs_cold": b / (c * 1e-3) / 1e9, "frac_hbm_cold": b / (c * 1e-3) / 1e9 / hbm_peak,
+                        "us_warm": warm * 1e3, "gbs_warm": b / (warm * 1e-3) / 1e9}
+    return out
+
+
 def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
     """BLAS-2 kernels inside running Davidson steps at a config whose basis is far larger than L2."""
     import torch
@@ -392,6 +428,10 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    try:
+        gt_probe = gemv_trans_probe(plan, V, W, flush, hbm_peak)
+    except Exception as e:
+        gt_probe = {"error": repr(e)}
     dav_large = None
     if world == 1 and not args.no_large:
         try:
@@ -440,7 +480,7 @@ def run_ours(args):
                          "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
                          "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
                          "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
-            "davidson_hbm": dav_large, "hpsi_curve": curve,
+            "davidson_hbm": dav_large, "gemv_trans": gt_probe, "hpsi_curve": curve,
             "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
     print(json.dumps(line), flush=True)
     if dist is not None:
