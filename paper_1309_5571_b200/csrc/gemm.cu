@@ -170,7 +170,8 @@ template <int STAGES, int MINB, int MODE>
 __global__ void __launch_bounds__(THREADS, MINB)
 grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restrict__ items, BasePtrs bases,
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
-                    const int *__restrict__ done_flag, int xvec, int yvec, unsigned long long *__restrict__ trace) {
+                    const int *__restrict__ done_flag, int xvec, int yvec, unsigned long long *__restrict__ trace,
+                    Prefetch pf) {
     if (done_flag && *done_flag) return;
     extern __shared__ __align__(16) double smem[];
     double *sPbase = smem;
@@ -352,6 +353,18 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             }
         }
     }
+    if (pf.base && ticket >= pf.first_ticket) {
+        // side job of the last CTAs in ticket order (done when their unit is done: the launch is draining): L2 prefetch of one slice
+        // of the rows the next kernel streams first; fire and forget, 128-byte lines
+        const long long lines = (pf.rows + 15) >> 4;
+        const int slice = ticket - pf.first_ticket;
+        const long long l0 = lines * slice / pf.n_ctas, l1 = lines * (slice + 1) / pf.n_ctas;
+        for (int c = 0; c < pf.cols; c++) {
+            const double *col = pf.base + (long long)c * pf.ld;
+            for (long long l = l0 + tid; l < l1; l += THREADS)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(col + (l << 4)));
+        }
+    }
     // publish: this tile of a T block is complete (release: every thread's stores, then the counter);
     // units that publish nothing skip the fence
     if (writes_c && u.signal >= 0) __threadfence();
@@ -375,7 +388,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
 typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int, int,
-                        unsigned long long *);
+                        unsigned long long *, Prefetch);
 struct Variant { const char *name; gemm_fn fn; int smem; };
 static const Variant kVariants[] = {
     {"s3b4m2", grouped_gemm_kernel<3, 4, 2>, smem_bytes(3)},   // default: measured best at cfg3 / 5a / 5b / 4096 sweep
@@ -396,7 +409,7 @@ cudaError_t gemm_kernel_setup() {
     return cudaSuccess;
 }
 
-int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st) {
+int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in) {
     BasePtrs b;
     b.p[BASE_X] = const_cast<double *>(x);
     b.p[BASE_Y] = y;
@@ -410,8 +423,14 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
     if (n_units > 0) {
         const int xvec = ((reinterpret_cast<uintptr_t>(x) & 15) == 0) ? 1 : 0;
         const int yvec = ((reinterpret_cast<uintptr_t>(y) & 15) == 0) ? 1 : 0;
+        Prefetch pf;
+        if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) {
+            pf = *pf_in;
+            pf.n_ctas = std::min(n_units, 4 * p->sm_count);
+            pf.first_ticket = n_units - pf.n_ctas;
+        }
         g_variant->fn<<<n_units, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
-                                                                 p->n_deps, done_flag, xvec, yvec, p->trace);
+                                                                 p->n_deps, done_flag, xvec, yvec, p->trace, pf);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

@@ -140,7 +140,10 @@ int dav_enqueue_step(Plan *p, double *V, double *W, long long ldv, int k, cudaSt
 int dav_ritz(Plan *p, const double *V, long long ldv, int k, double *x_out, cudaStream_t st);
 int dav_gemv_trans(Plan *p, const double *V, long long ldv, int k, const double *w, double *out, cudaStream_t st);
 int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s, double *t, double *nrm2, cudaStream_t st);
-int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st);
+// Optional side job of the last CTAs of an apply: pull the first `rows` rows of `cols` columns (column stride `ld`)
+// into L2 for the kernel that follows (the Davidson basis for line 3), while the launch drains and HBM is idle.
+struct Prefetch { const double *base = nullptr; long long ld = 0, rows = 0; int cols = 0, first_ticket = 0, n_ctas = 0; };
+int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf = nullptr);
 
 // probe.cu
 int probe_fp64(int kind, int reps, double *tflops, cudaStream_t st);
