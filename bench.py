@@ -407,15 +407,16 @@ def run_ours(args):
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
-    traffic = None
+    traffic, traffic_note = None, None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.config, {}).get("grouped_gemm_dram_bytes_per_launch")
+        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.config, {})
+        traffic, traffic_note = tj.get("grouped_gemm_dram_bytes_per_launch"), tj.get("note")
     except Exception:
         pass
     achieved = st["flop_per_apply"] / (gemm_ms * 1e-3) / 1e12
     roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (DMMA.8x8x4; 1 launch per step: stage-1 and stage-2 units in ticket order)",
                 "achieved": achieved, "peak": max(dmma_peak, dfma_peak), "unit": "TFLOP/s",
-                "frac": achieved / max(dmma_peak, dfma_peak), "traffic": traffic,
+                "frac": achieved / max(dmma_peak, dfma_peak), "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": "measured live: register-only DMMA.8x8x4 issue-rate probe (dmrg_probe_fp64_peak); "
                                f"DFMA probe {dfma_peak:.1f}; nominal 148 SM x 128 FLOP/clk x 1.965 GHz = 37.2",
                 "flop_per_launch": st["flop_per_apply"], "ms_per_launch": gemm_ms}
