@@ -232,7 +232,7 @@ def test_not_converged_and_breakdown_codes(lib):
 
 
 def test_small_eig_fast_path_equals_jacobi_fallback():
-    """Line 4 has two implementations in one kernel: the arrowhead secular solve (warm start, k >= 5) and the Jacobi
+    """Line 4 has two implementations in one kernel: the arrowhead secular solve (warm start, k >= 3) and the Jacobi
     sweeps it falls back to.  DMRG_EIG_FAST is read once per process, so each mode runs in its own process; the
     lambda / ||r|| trajectories from the deterministic start must agree to rounding."""
     import json, os, subprocess, sys
