@@ -398,3 +398,41 @@ def test_trajectory_parity_fuzz(lib, seed):
         # the same eigenpair (the first 45 iterations above are compared one by one); only guard against a stall
         assert full["iters"] / 1.6 - 10 <= iters <= full["iters"] * 1.6 + 10, (seed, k_max, reorth, iters, full["iters"])
     plan.close()
+
+
+@pytest.mark.parametrize("pad", [1, 3])
+def test_odd_column_stride_takes_the_scalar_path_and_agrees(lib, pad):
+    """With an odd column stride the columns of V, W are only 8-byte aligned: the Davidson kernels fall back to their
+    64-bit-load instantiations, the fused residual pass and the 16-byte paths are off (include/dmrg_b200.h: 'ldv even
+    keeps 16-byte vector loads').  30 iterations (through a restart at k_max = 7) must follow the 16-byte-path run to
+    rounding, and the enqueue-only / host-buffer calls must work on that path too."""
+    import torch
+    p = SMALL["heis_syn_m300_ragged"]()
+    plan = lib.Plan(p, k_max=7, tol=1e-12)
+    n = plan.n
+    odd = n + pad if (n + pad) % 2 == 1 else n + pad + 1
+    Va, Wa = plan.new_basis()
+    Vb, Wb = plan.new_basis(ldv=odd)
+    plan.davidson_init(Va, Wa, start_at_argmin_diag=True)
+    ka, ref = 1, []
+    for _ in range(30):
+        ka, lam, rho, conv = plan.davidson_step(Va, Wa, ka)
+        ref.append((ka, lam, rho))
+    plan.davidson_init(Vb, Wb, start_at_argmin_diag=True)
+    hw = torch.empty(n, dtype=torch.float64).pin_memory()
+    kb = 1
+    for i in range(30):
+        if i % 3 == 0:
+            kb, lam, rho, conv = plan.davidson_step(Vb, Wb, kb)
+        elif i % 3 == 1:
+            kb = plan.davidson_enqueue(Vb, Wb, kb)
+            lam, rho, conv, _ = plan.davidson_poll()
+        else:
+            kprev = kb
+            kb, lam, rho, conv = plan.davidson_step_host(Vb, Wb, kb, None, hw)
+            if kprev != 7:          # a restart step rewrites W(:,0..1) after the copy
+                assert torch.equal(hw, Wb[kprev - 1, :n].cpu())
+        assert kb == ref[i][0]
+        assert abs(lam - ref[i][1]) <= 1e-11 and abs(rho - ref[i][2]) <= 1e-9 + 1e-6 * ref[i][2], (i, lam, ref[i])
+    assert float((Va[:ka, :n] - Vb[:kb, :n]).abs().max()) <= 1e-7
+    plan.close()
