@@ -141,11 +141,13 @@ def test_trajectory_parity_small(lib, name, k_max, iters):
         assert abs(abs(x @ ores["x"]) - 1.0) <= OVERLAP_DEF
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg3"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg3", "cfg5a"])
 def test_trajectory_parity_full_config(lib, name):
-    """BASELINE.json configs at full size, deterministic start, fixed iteration count (A20)."""
+    """BASELINE.json configs 2-5 at full size, deterministic start (D), the iteration count and basis limit each
+    config names (50 / 50 / 100 with k_max = 24 / 100 with k_max = 32), compared iteration by iteration (A20)."""
     from dmrg_inputs import CONFIGS
-    iters = {"cfg2": 50, "cfg4": 50, "cfg3": 40}[name]
+    iters = CONFIGS[name]["iters"]
+    assert iters == {"cfg2": 50, "cfg4": 50, "cfg3": 100, "cfg5a": 100}[name]
     hist, ores, _ = _trajectory(lib, full_config(name), CONFIGS[name]["k_max"], iters)
     assert len(hist) == len(ores["history"]) == iters
     for (lg, rg), (lo, ro) in zip(hist, ores["history"]):
@@ -182,9 +184,10 @@ def test_cfg1_eigenpair_vs_exact_diagonalisation(lib):
     plan.close()
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg3", "cfg5a"])
 def test_converged_eigenpair_full_config(lib, name):
-    """Converged lowest eigenpair at full size, random start (R), vs the oracle's own Davidson run."""
+    """Converged lowest eigenpair at full size, random start (R), vs the oracle's own Davidson run to the same
+    tolerance: |d lambda| <= 1e-9, overlap >= 1 - 1e-6 (north_star), configs 2, 3, 4 and 5a."""
     from dmrg_inputs import CONFIGS
     p = full_config(name)
     lay = rec.Layout(p)
@@ -199,6 +202,23 @@ def test_converged_eigenpair_full_config(lib, name):
     assert abs(lam - ores["lam"]) <= LAMBDA_ATOL
     assert abs(x.cpu().numpy() @ ores["x"]) >= 1 - OVERLAP_DEF
     plan.close()
+
+
+@pytest.mark.slow
+def test_lockstep_cfg5b(lib):
+    """Paper-scale config 5b (n ~ 1.5e7; SURVEY 8(d) row 5b "H*x + lock-step parity"): five single steps from the GPU's
+    own state, each handed to ONE oracle step -- k = 1, 2, 3, the restart step at k = k_max (k_max reduced to 4 so that
+    the host copy of V, W stays ~1 GB) and the step after it."""
+    worst = _lockstep(lib, full_config("cfg5b"), 4, 5, None)
+    assert worst["lam"] <= LAMBDA_ATOL and worst["rho"] <= 1.0 and worst["B"] <= 1e-10 and worst["v"] <= 1e-7, worst
+
+
+def test_kmax32_lockstep_cfg5a(lib):
+    """k_max = 32 (the basis limit config 5 names) at n ~ 9e5 in lock step from the seeded random start (R): 36 steps,
+    i.e. every basis size 1..32, the restart step and three steps after it."""
+    p = full_config("cfg5a")
+    worst = _lockstep(lib, p, 32, 36, random_vector(rec.Layout(p).n, vector_seed("cfg5a", "start")))
+    assert worst["lam"] <= LAMBDA_ATOL and worst["rho"] <= 1.0 and worst["B"] <= 1e-10 and worst["v"] <= 1e-7, worst
 
 
 def test_cfg3_converged_eigenpair_properties(lib):

@@ -110,9 +110,12 @@ def test_record_and_flop_counts_config1():
     assert gemms == 52
     # A24 by hand for dims 1,6,15,20,15,6,1 (pairs (q,-q)):
     d = [1, 6, 15, 20, 15, 6, 1]
-    f = sum(2 * d[i] ** 2 * d[6 - i] + 2 * d[i] * d[6 - i] ** 2 for i in range(7))            # H_L(x)I, I(x)H_R
-
-    assert rec.flop_count(p, lay) == 220928
+    f_id = sum(2 * d[i] ** 2 * d[6 - i] + 2 * d[i] * d[6 - i] ** 2 for i in range(7))         # H_L(x)I, I(x)H_R: one GEMM each
+    f_zz = sum(2 * d[i] ** 2 * d[6 - i] + 2 * d[i] * d[6 - i] ** 2 for i in range(7))         # Sz(x)Sz: two GEMMs, same shapes
+    # S+(x)S- and S-(x)S+ move pair (i, 6-i) to (i+1, 5-i) and back; both association orders cost 2ab(a+b)
+    f_pm = 2 * sum(2 * d[i] * d[i + 1] * (d[i] + d[i + 1]) for i in range(6))
+    assert (f_id, f_zz, f_pm) == (60736, 60736, 99456)
+    assert rec.flop_count(p, lay) == f_id + f_zz + f_pm == 220928
 
 
 def test_empty_sector_and_no_pair():
