@@ -349,9 +349,10 @@ class Plan:
         return ms
 
     def unit_trace(self):
-        """Diagnostics (plan created with DMRG_TRACE set): (n_units, 4) uint64 array of the last apply."""
+        """Diagnostics (plan created with DMRG_TRACE set): (rows, 4) uint64 array of the last apply: one row per work
+        unit in ticket order, then one row of phase stamps per CTA slot (include/dmrg_b200.h)."""
         st = self.stats()
-        cap = st["stage1_units"] + st["stage2_units"]
+        cap = st["stage1_units"] + st["stage2_units"] + 8 * 256
         buf = np.zeros((max(cap, 1), 4), dtype=np.uint64)
         nu = C.c_int32()
         self._check(self._lib.dmrg_get_unit_trace(self._h, buf.ctypes.data_as(C.POINTER(C.c_uint64)), cap, C.byref(nu)))

@@ -19,6 +19,8 @@ int read_state(Plan *p, cudaStream_t st, bool full = true) {
                                     sizeof(DavState) - off, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, std::string("state read-back: ") + cudaGetErrorString(e));
+    if (p->state_host->gemm_error)
+        return fail(p, DMRG_E_CUDA, "projection: a dependency wait gave up (launches of one plan interleaved on two streams, or a lost launch)");
     return DMRG_OK;
 }
 void ensure_timing(Plan *p) {

@@ -1,25 +1,30 @@
-// gemm.cu -- grouped FP64 tensor-core (DMMA) kernel of the projection: ONE launch per apply.
+// gemm.cu -- grouped FP64 tensor-core (DMMA) kernel of the projection: ONE persistent launch per apply.
 //
-// Computes, for every work unit, a 64x64 tile of  C = sum_items P_item * Q_item  (row-major
-// operands, K concatenated over the unit's items) -- Eq. 11 of the paper,
+// Computes, for every work unit, a 64x64 tile of  C = sum_items P_item * Q_item  (K concatenated over the
+// unit's items) -- Eq. 11 of the paper,
 //     X'_jl += A_{i->j} X_ik B_{k->l}^T
-// with the sum over the records of one output realised as ONE long-K
-// product so that nothing is accumulated through memory and no atomics touch the data.
+// with the sum over the records of one output realised as ONE long-K product so that
+// nothing is accumulated through memory and no atomics touch the data.
 //
-// Both stages of every record run in the same launch: units are handed out through a ticket
-// counter in a fixed order -- all stage-1 units (T = X B^T or T = A X) first, then the stage-2
-// units (X' tiles) -- and a stage-2 unit waits, item by item, on the "T block complete" counter of
-// the stage-1 task that produces its operand.  A waiting unit only ever waits on units with a
-// smaller ticket, which are running or finished, so the wait always ends.  This is the paper's
-// "one stream per output, depth-first issue" (Alg. 7) without a launch boundary.
+// Both stages of every record run in the same launch: units are handed out through a ticket counter in a
+// fixed order -- all stage-1 units (T = X B^T or T = A X) first, then the stage-2 units (X' tiles) -- and a
+// stage-2 unit waits, item by item, on the "T block complete" counter of the stage-1 task that produces its
+// operand.  A waiting unit only ever waits on units with a smaller ticket, which are running or finished, so
+// the wait always ends.  This is the paper's "one stream per output, depth-first issue" (Alg. 7,
+// PAPER.md:L432-445) without a launch boundary.
 //
-// sm_100a specifics: FP64 has no tcgen05/TMEM path (ptxas rejects .kind::f64); the FP64 tensor
-// instruction is mma.sync m8n8k4 -> SASS DMMA.8x8x4, measured at 37.0 TFLOP/s on B200 (the
-// DFMA pipe gives 33.9).  Operands are staged through shared memory with a 3-stage cp.async
-// (LDGSTS) pipeline whose per-thread source pointers are bumped, not recomputed, per k-tile;
-// padded rows (+4 doubles) make both fragment loads bank-conflict free.  Ragged edges and odd row
-// strides are handled by zero-filling cp.async (src-size < cp-size); a warp whose 32x32 tile holds data only in
-// its first 16 rows and/or columns runs a 2x4, 4x2 or 2x2 block of DMMA tiles instead of 4x4 (no predicates).
+// sm_100a specifics.  FP64 has no tcgen05/TMEM path (ptxas rejects .kind::f64); the FP64 tensor instruction is
+// mma.sync m8n8k4 -> SASS DMMA.8x8x4 (one per 16 clocks per SM sub-partition: 37 TFLOP/s per chip).
+// The kernel is WARP-SPECIALISED and PERSISTENT: each CTA = 4 consumer warps (2x2, warp tile 32x32, register
+// accumulators) + 1 producer warp, 3 CTAs per SM, a ring of STAGES k-tiles (64x16 of P, 16x64 of Q; 16 KB) with one
+// "full" and one "empty" mbarrier per stage -- there is no CTA-wide barrier in the main loop, and the producer
+// runs ahead across unit boundaries (the next unit's first k-tiles land while the consumers are in the epilogue).
+// Every operand (the repacked operator pool, the T workspace and -- after phase 0 of the kernel, in which all CTAs
+// rewrite the caller's vector -- the input vector) is stored as 8 KB TILE IMAGES: the exact, bank-conflict-free (XOR-swizzled)
+// shared-memory picture of one k-tile, edges zero-padded, so that a k-tile of an operand is staged by ONE bulk
+// asynchronous copy of the TMA unit (cp.async.bulk, SASS UBLKCP) that signals the stage's mbarrier with complete_tx.
+// One elected producer thread issues two such copies per k-tile; dependency waits are the producer's: the consumers
+// keep draining the ring meanwhile.
 #include <cstdlib>
 #include <string>
 #include "internal.h"
@@ -28,24 +33,61 @@ namespace dmrg {
 
 namespace {
 
-constexpr int THREADS = 128;               // 4 warps, 2x2, warp tile 32x32
-constexpr int LDP = BK + 4;                // 20 doubles: rows land on distinct bank groups
-constexpr int LDQ = BN + 4;                // 68
-constexpr int P_STAGE = BM * LDP;          // doubles
-constexpr int Q_STAGE = BK * LDQ;
-constexpr int smem_bytes(int stages) { return stages * (P_STAGE + Q_STAGE) * 8; }
+constexpr int CONSUMERS = CWARPS * 32;     // consumer warps: 2 (M) x CWARPS/2 (N); warp tile 32 x (128 / CWARPS)
+constexpr int THREADS = CONSUMERS + 32;    // + 1 producer warp
+constexpr int NJW = 16 / CWARPS;           // 8-column sub-tiles per warp: 4 (four warps) or 2 (eight warps)
+static_assert(CWARPS == 4 || CWARPS == 8, "consumer layout");
+constexpr int STAGE_DOUBLES = 2 * IMG;     // P image + Q image
+constexpr int UNIT_WORDS = (int)(sizeof(GemmUnit) / 4);
+static_assert(UNIT_WORDS <= 32, "one lane per word of the unit descriptor");
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *g, int src_bytes) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(src_bytes));
+enum : int { F_DATA = 1, F_LAST = 2, F_EXIT = 4, F_FIRST = 8, F_REDUCE = 16, F_HALF = 32 };
+constexpr int PUBLISH_DELAY = 2;           // stages a consumer warp works on before it fences and signals a finished tile
+struct StageHdr {
+    int flags, ticket, ext_m, ext_n;       // ext: rows / columns of the 64x64 tile that hold data
+    int rot, pad[3];                       // sub-tile rotation of the unit (see the consumers)
+    int u[UNIT_WORDS];                     // the unit descriptor (valid in the unit's last stage: epilogue)
+};
+constexpr int smem_bytes(int stages) { return stages * (STAGE_DOUBLES * 8 + (int)sizeof(StageHdr) + 16) + 128; }
+
+// ---- PTX helpers
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void cp_async8(void *smem, const void *g, int src_bytes) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(g), "r"(src_bytes));
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// one 8 KB tile image, global -> shared, completion counted in bytes on the stage's mbarrier (TMA unit, UBLKCP)
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;\n" ::: "memory"); }
+__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -67,94 +109,47 @@ __device__ __forceinline__ unsigned smid() {
     return s;
 }
 
-
-// Per-thread producer state of the current item: source pointers of this thread's first chunk in the
-// P tile (BM x BK) and the Q tile (BK x BN), bumped by one k-tile after every produce.
-//   16-byte mode: P chunk (row tid/8 + 16 s, col 2 (tid%8)), s < 4;  Q chunk (row tid/32 + 4 s, col 2 (tid%32)), s < 4
-//    8-byte mode: P chunk (row tid/16 + 8 s, col tid%16),     s < 8;  Q chunk (row tid/64 + 2 s, col tid%64),     s < 8
+// ---------------------------------------------------------------- producer warp
 struct Producer {
-    const double *pP, *pQ;     // bumped
-    const double *P0, *Q0;     // item bases (a legal address for zero-byte copies)
-    int stepP, stepQ;          // element distance between consecutive s-chunks
+    const double *pP, *pQ;     // the next k-tile's images, bumped by one image per k-tile
     int K, k0;                 // item K; k0 of the next tile to produce
-    bool pv, qv;
 };
 
-__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, bool xvec,
-                                           int m0, int n0, int k0, int tid, const int *ctrl) {
+__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, int m0, int n0, int k0,
+                                           int lane, const int *ctrl, int *err) {
     const int dep = it->dep;
     if (dep >= 0) {            // operand is a T block of this launch: wait until all its tiles are written
-        const int need = it->dep_need;
-        const int *c = ctrl + CTRL_DEP0 + dep;
-        while (ld_acquire(c) < need) __nanosleep(64);
+        if (lane == 0) {
+            const int need = it->dep_need;
+            const int *c = ctrl + CTRL_DEP0 + dep;
+            long long spins = 0;
+            while (ld_acquire(c) < need) {
+                __nanosleep(32);
+                if (++spins > (1ll << 26)) { atomicExch(err, 1); break; }   // seconds: a lost launch, not a slow one
+            }
+        }
+        __syncwarp();
+        fence_proxy_async();   // the T images were written through the generic proxy, the bulk copy reads through the async one
     }
-    const int pb = it->p_base, qb = it->q_base;
-    pr.P0 = bases[pb] + it->p_off; pr.Q0 = bases[qb] + it->q_off;
     pr.K = it->K; pr.k0 = k0;
-    pr.pv = it->p_vec2 && (pb != BASE_X || xvec);
-    pr.qv = it->q_vec2 && (qb != BASE_X || xvec);
-    const int ldp = it->ldp, ldq = it->ldq;
-    if (pr.pv) { pr.pP = pr.P0 + (long long)(m0 + (tid >> 3)) * ldp + k0 + 2 * (tid & 7); pr.stepP = 16 * ldp; }
-    else       { pr.pP = pr.P0 + (long long)(m0 + (tid >> 4)) * ldp + k0 + (tid & 15);    pr.stepP = 8 * ldp; }
-    if (pr.qv) { pr.pQ = pr.Q0 + (long long)(k0 + (tid >> 5)) * ldq + n0 + 2 * (tid & 31); pr.stepQ = 4 * ldq; }
-    else       { pr.pQ = pr.Q0 + (long long)(k0 + (tid >> 6)) * ldq + n0 + (tid & 63);     pr.stepQ = 2 * ldq; }
+    const int KT = (pr.K + BK - 1) / BK;
+    pr.pP = bases[it->p_base] + it->p_off + ((long long)(m0 / BM) * KT + k0 / BK) * IMG;
+    pr.pQ = bases[it->q_base] + it->q_off + ((long long)(n0 / BN) * KT + k0 / BK) * IMG;
 }
 
-// rowmask16 / rowmask8: bit s set if this thread's s-th P chunk row is inside M (fixed per unit);
-// colb16 / colb8: bytes of this thread's Q chunk that lie inside N (fixed per unit).
-__device__ __forceinline__ void produce_tile(Producer &pr, double *sP, double *sQ, int tid,
-                                             unsigned rowmask16, unsigned rowmask8, int colb16, int colb8) {
-    const int K = pr.K, k0 = pr.k0;
-    if (pr.pv) {
-        const int kb = max(0, min(K - (k0 + 2 * (tid & 7)), 2)) * 8;
-        double *d = sP + (tid >> 3) * LDP + 2 * (tid & 7);
-#pragma unroll
-        for (int s = 0; s < 4; s++) {
-            const int bytes = ((rowmask16 >> s) & 1) ? kb : 0;
-            cp_async16(d + s * 16 * LDP, bytes ? pr.pP + (long long)s * pr.stepP : pr.P0, bytes);
-        }
-    } else {
-        const int kb = (k0 + (tid & 15) < K) ? 8 : 0;
-        double *d = sP + (tid >> 4) * LDP + (tid & 15);
-#pragma unroll
-        for (int s = 0; s < 8; s++) {
-            const int bytes = ((rowmask8 >> s) & 1) ? kb : 0;
-            cp_async8(d + s * 8 * LDP, bytes ? pr.pP + (long long)s * pr.stepP : pr.P0, bytes);
-        }
-    }
-    if (pr.qv) {
-        double *d = sQ + (tid >> 5) * LDQ + 2 * (tid & 31);
-        const int kr = K - k0 - (tid >> 5);          // rows left from this thread's first chunk row on
-#pragma unroll
-        for (int s = 0; s < 4; s++) {
-            const int bytes = (4 * s < kr) ? colb16 : 0;
-            cp_async16(d + s * 4 * LDQ, bytes ? pr.pQ + (long long)s * pr.stepQ : pr.Q0, bytes);
-        }
-        pr.pQ += 4 * (long long)pr.stepQ;            // BK rows = 4 steps of 4 rows
-    } else {
-        double *d = sQ + (tid >> 6) * LDQ + (tid & 63);
-        const int kr = K - k0 - (tid >> 6);
-#pragma unroll
-        for (int s = 0; s < 8; s++) {
-            const int bytes = (2 * s < kr) ? colb8 : 0;
-            cp_async8(d + s * 2 * LDQ, bytes ? pr.pQ + (long long)s * pr.stepQ : pr.Q0, bytes);
-        }
-        pr.pQ += 8 * (long long)pr.stepQ;            // BK rows = 8 steps of 2 rows
-    }
-    pr.pP += BK;
-    pr.k0 = k0 + BK;
-}
-
+// ---------------------------------------------------------------- consumer warps
 // One k-tile of the warp tile restricted to its first MI x NJ sub-tiles (compile-time bounds: no predicates).
+// offA[k4] / offB[j]: this lane's swizzled element offsets inside the P / Q image (constant over the kernel).
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_ktile(double (&acc)[4][4][2], const double *pa, const double *pb) {
+__device__ __forceinline__ void mma_ktile(double (&acc)[4][NJW][2], const double *sP, const double *sQ,
+                                          const int (&offA)[4], const int (&offB)[NJW]) {
 #pragma unroll
     for (int k4 = 0; k4 < BK / 4; k4++) {
         double a[MI], b[NJ];
 #pragma unroll
-        for (int i = 0; i < MI; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
+        for (int i = 0; i < MI; i++) a[i] = sP[i * 8 * BK + offA[k4]];
 #pragma unroll
-        for (int j = 0; j < NJ; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
+        for (int j = 0; j < NJ; j++) b[j] = sQ[k4 * 4 * BN + offB[j]];
 #pragma unroll
         for (int i = 0; i < MI; i++)
 #pragma unroll
@@ -162,224 +157,388 @@ __device__ __forceinline__ void mma_ktile(double (&acc)[4][4][2], const double *
     }
 }
 
-// MODE 0: every DMMA of the 64x64x16 tile is issued (padding multiplies zeros);
-// MODE 1: sub-tiles that hold only padding are skipped (8-granular in M, N; 4-granular in K);
-// MODE 2: warp tiles whose data fits in the first 2 sub-tile rows / columns run a 2x4, 4x2 or 2x2 DMMA block
-//         (16-granular, no predicates), empty warp tiles run nothing.
-template <int STAGES, int MINB, int MODE>
+// Phase 0: this CTA's contiguous share [lo, hi) of the caller's vector -> tile images (internal.h), written to the P images
+// (X_ik as M x K) and to the Q images (X_ik as K x N) of the segment each element falls in.  Up to twelve independent loads per
+// thread are in flight before the first store; scalar loads, any alignment of x.
+__device__ __forceinline__ void ximg_share(const XSeg *__restrict__ segs, int n_segs, const double *__restrict__ x,
+                                           long long lo, long long hi, double *__restrict__ xp, double *__restrict__ xq, int tid) {
+    constexpr int U = 12;     // cfg 3 / 5a: a share is ~9-11 elements per thread -> every load of a share is in flight at once
+    if (lo + tid >= hi) return;
+    int a = 0;                                               // last segment with seg_off <= this thread's first element
+    {
+        int b = n_segs - 1;
+        const long long e0 = lo + tid;
+        while (a < b) { const int m = (a + b + 1) >> 1; if (segs[m].seg_off <= e0) a = m; else b = m - 1; }
+    }
+    XSeg sg = segs[a];
+    long long next_off = (a + 1 < n_segs) ? segs[a + 1].seg_off : (long long)0x7fffffffffffffffll;
+    for (long long base = lo + tid; base < hi; base += (long long)U * THREADS) {
+        double v[U];
+#pragma unroll
+        for (int q = 0; q < U; q++) { const long long e = base + (long long)q * THREADS; v[q] = e < hi ? x[e] : 0.0; }
+#pragma unroll
+        for (int q = 0; q < U; q++) {
+            const long long e = base + (long long)q * THREADS;
+            if (e >= hi) break;
+            while (e >= next_off) {                          // this thread's elements ascend: walk, do not search
+                a++; sg = segs[a];
+                next_off = (a + 1 < n_segs) ? segs[a + 1].seg_off : (long long)0x7fffffffffffffffll;
+            }
+            const int w = (int)(e - sg.seg_off), r = w / sg.dk, c = w - r * sg.dk;
+            const int KTp = (sg.dk + BK - 1) / BK, KTq = (sg.di + BK - 1) / BK;
+            xp[sg.xp_off + ((long long)(r / BM) * KTp + c / BK) * IMG + img_p_index(r % BM, c % BK)] = v[q];
+            xq[sg.xq_off + ((long long)(c / BN) * KTq + r / BK) * IMG + img_q_index(r % BK, c % BN)] = v[q];
+        }
+    }
+}
+
+template <int STAGES, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restrict__ items, BasePtrs bases,
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
-                    const int *__restrict__ done_flag, int xvec, int yvec, unsigned long long *__restrict__ trace,
-                    Prefetch pf) {
+                    const int *__restrict__ done_flag, int yvec, unsigned long long *__restrict__ trace,
+                    Prefetch pf, int *__restrict__ err, const XSeg *__restrict__ xsegs, int n_xsegs,
+                    const double *__restrict__ x, long long n) {
     if (done_flag && *done_flag) return;
-    extern __shared__ __align__(16) double smem[];
-    double *sPbase = smem;
-    double *sQbase = smem + STAGES * P_STAGE;
-    __shared__ int s_ticket, s_is_last;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *stage_base = reinterpret_cast<double *>(smem_raw);
+    StageHdr *hdrs = reinterpret_cast<StageHdr *>(smem_raw + (size_t)STAGES * STAGE_DOUBLES * 8);
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(hdrs + STAGES);     // full[STAGES], empty[STAGES]
+    __shared__ double *s_base[BASE_COUNT];      // dynamically indexed: shared memory, not a local-memory copy of the parameter
+    __shared__ int s_is_last;                   // end of the launch only
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_ticket = atomicAdd(&ctrl[CTRL_TICKET], 1);
-    __syncthreads();
-    const int ticket = s_ticket;
-    // the unit descriptor lives in shared memory (read on demand) rather than in ~20 registers across the main loop
-    __shared__ GemmUnit s_u;
-    __shared__ double *s_base[BASE_COUNT];      // dynamically indexed: shared memory, not a local-memory copy of the parameter
-    if (tid < (int)(sizeof(GemmUnit) / 4)) reinterpret_cast<int *>(&s_u)[tid] = reinterpret_cast<const int *>(units + ticket)[tid];
-    if (tid == 32) { s_base[BASE_X] = bases.p[BASE_X]; s_base[BASE_Y] = bases.p[BASE_Y]; s_base[BASE_T] = bases.p[BASE_T]; s_base[BASE_POOL] = bases.p[BASE_POOL]; s_base[BASE_PART] = bases.p[BASE_PART]; }
-    __syncthreads();
-    const GemmUnit &u = s_u;
-    unsigned long long t_start = 0, t_main = 0;
-    if (trace && tid == 0) t_start = globaltimer();
-
-    const int wm = (warp & 1) * 32, wn = (warp >> 1) * 32;
-    const int g = lane >> 2, tg = lane & 3;
-    const GemmItem *uitems = items + u.item_begin;
-
-    double acc[4][4][2];
+    if (tid == 0) {
 #pragma unroll
-    for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int j = 0; j < 4; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
-
-    // per-unit constants of the producer
-    unsigned rowmask16 = 0, rowmask8 = 0;
-#pragma unroll
-    for (int s = 0; s < 4; s++) if (u.m0 + (tid >> 3) + 16 * s < u.M) rowmask16 |= 1u << s;
-#pragma unroll
-    for (int s = 0; s < 8; s++) if (u.m0 + (tid >> 4) + 8 * s < u.M) rowmask8 |= 1u << s;
-    const int colb16 = max(0, min(u.N - (u.n0 + 2 * (tid & 31)), 2)) * 8;
-    const int colb8 = (u.n0 + (tid & 63) < u.N) ? 8 : 0;
-
-    // producer cursor: walk to kt_begin; the consumer follows the same sequence STAGES-1 tiles behind
-    int p_item = u.item0, p_k0 = u.k00;      // resolved by the planner
-    const int KT = u.kt_count;
-    Producer pr{};
-    if (KT > 0) begin_item(pr, uitems + p_item, s_base, xvec != 0, u.m0, u.n0, p_k0, tid, ctrl);
-    int c_item = p_item, c_k0 = p_k0, c_K = pr.K;
-    auto produce = [&](int stage) {
-        produce_tile(pr, sPbase + stage * P_STAGE, sQbase + stage * Q_STAGE, tid, rowmask16, rowmask8, colb16, colb8);
-        if (pr.k0 >= pr.K) {
-            p_item++;
-            if (p_item < u.item_count) begin_item(pr, uitems + p_item, s_base, xvec != 0, u.m0, u.n0, 0, tid, ctrl);
+        for (int s = 0; s < STAGES; s++) {
+            mbar_init(smem_u32(bars + s), 1);             // the producer's arrive(.expect_tx); the bytes complete the phase
+            mbar_init(smem_u32(bars + STAGES + s), CWARPS);   // one arrival per consumer warp
         }
-    };
-    // sub-tiles of this warp that hold real rows / columns (8-granular): padding issues no DMMA
-    const int mi = min(max(u.M - (u.m0 + wm) + 7, 0) >> 3, 4);
-    const int nj = min(max(u.N - (u.n0 + wn) + 7, 0) >> 3, 4);
-    const bool full_warp_tile = (mi == 4 && nj == 4);
-
-    int issued = 0;
-#pragma unroll
-    for (int s = 0; s < STAGES - 1; s++) {
-        if (issued < KT) { produce(s); issued++; }
-        cp_async_commit();
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    for (int t = 0; t < KT; t++) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        if (issued < KT) { produce(issued % STAGES); issued++; }
-        cp_async_commit();
-        const int nk4 = (min(c_K - c_k0, BK) + 3) >> 2;    // k4-steps with real K in this tile
-        c_k0 += BK;
-        if (c_k0 >= c_K) {
-            c_item++; c_k0 = 0;
-            if (c_item < u.item_count) c_K = uitems[c_item].K;
+    if (tid < BASE_COUNT) s_base[tid] = bases.p[tid];
+    unsigned long long *ctr = trace ? trace + 4ull * n_units + 4ull * blockIdx.x : nullptr;   // per-CTA phase stamps (diagnostics)
+    if (ctr && tid == 0) ctr[0] = globaltimer();
+    // Phase 0: the caller's vector -> tile images (both operand roles), shared out over all CTAs; a CTA publishes its share
+    // (CTRL_XREADY) and the producers wait for all shares before their first copy.  Every CTA of the grid is resident
+    // (the grid is one wave), and each writes its share before it waits for anything.
+    {
+        const long long share = (n + gridDim.x - 1) / gridDim.x, lo = share * blockIdx.x;
+        const XSeg *segs = xsegs;
+        if ((size_t)n_xsegs * sizeof(XSeg) <= (size_t)STAGES * STAGE_DOUBLES * 8) {     // the segment table fits the (still idle) ring
+            int *dst = reinterpret_cast<int *>(smem_raw);
+            const int *src = reinterpret_cast<const int *>(xsegs);
+            for (int e = tid; e < n_xsegs * (int)(sizeof(XSeg) / 4); e += THREADS) dst[e] = src[e];
+            __syncthreads();
+            segs = reinterpret_cast<const XSeg *>(smem_raw);
         }
-        const double *pa = sPbase + (t % STAGES) * P_STAGE + (wm + g) * LDP + tg;
-        const double *pb = sQbase + (t % STAGES) * Q_STAGE + tg * LDQ + wn + g;
-        if (MODE == 2) {
-            if (mi > 2 && nj > 2) mma_ktile<4, 4>(acc, pa, pb);
-            else if (mi > 2 && nj > 0) mma_ktile<4, 2>(acc, pa, pb);
-            else if (mi > 0 && nj > 2) mma_ktile<2, 4>(acc, pa, pb);
-            else if (mi > 0 && nj > 0) mma_ktile<2, 2>(acc, pa, pb);
-        } else if (MODE == 0 || (full_warp_tile && nk4 == BK / 4)) {
-#pragma unroll
-            for (int k4 = 0; k4 < BK / 4; k4++) {
-                double a[4], b[4];
-#pragma unroll
-                for (int i = 0; i < 4; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
-#pragma unroll
-                for (int j = 0; j < 4; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
-#pragma unroll
-                for (int i = 0; i < 4; i++)
-#pragma unroll
-                    for (int j = 0; j < 4; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        ximg_share(segs, n_xsegs, x, lo, min(n, lo + share), bases.p[BASE_XP], bases.p[BASE_XQ], tid);
+    }
+    fence_proxy_async();
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) atomicAdd(&ctrl[CTRL_XREADY], 1);
+    if (ctr && tid == 0) ctr[1] = globaltimer();
+
+    if (warp == CONSUMERS / 32) {
+        // ================================================= producer
+        if (lane == 0) {
+            long long spins = 0;
+            while (ld_acquire(&ctrl[CTRL_XREADY]) < (int)gridDim.x) {
+                __nanosleep(32);
+                if (++spins > (1ll << 26)) { atomicExch(err, 1); break; }
             }
-        } else if (mi > 0 && nj > 0) {
-#pragma unroll
-            for (int k4 = 0; k4 < BK / 4; k4++) {
-                if (k4 < nk4) {
-                    double a[4], b[4];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) a[i] = pa[i * 8 * LDP + k4 * 4];
-#pragma unroll
-                    for (int j = 0; j < 4; j++) b[j] = pb[k4 * 4 * LDQ + j * 8];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        if (i < mi) {
-#pragma unroll
-                            for (int j = 0; j < 4; j++)
-                                if (j < nj) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        __syncwarp();
+        fence_proxy_async();
+        if (ctr && lane == 0) ctr[2] = globaltimer();
+        int g = 0;                                   // stages issued so far
+        auto acquire = [&]() {                       // waits until the consumers have released the stage; returns its index
+            const int s = g % STAGES;
+            if (g >= STAGES) mbar_wait(smem_u32(bars + STAGES + s), ((g / STAGES) & 1) ^ 1);
+            return s;
+        };
+        for (;;) {
+            int ticket = 0;
+            if (lane == 0) ticket = atomicAdd(&ctrl[CTRL_TICKET], 1);
+            ticket = __shfl_sync(0xffffffffu, ticket, 0);
+            if (ticket >= n_units) break;
+            const int uw = lane < UNIT_WORDS ? reinterpret_cast<const int *>(units + ticket)[lane] : 0;
+#define UFIELD(f) __shfl_sync(0xffffffffu, uw, (int)(offsetof(GemmUnit, f) / 4))
+            const int M = UFIELD(M), N = UFIELD(N), m0 = UFIELD(m0), n0 = UFIELD(n0);
+            (void)0;
+            const int item_begin = UFIELD(item_begin), item_count = UFIELD(item_count);
+            const int KT = UFIELD(kt_count);
+            int p_item = UFIELD(item0);
+            const int k00 = UFIELD(k00);
+            const int n_split = UFIELD(n_split), split_idx = UFIELD(split_idx), tile_id = UFIELD(tile_id);
+            const int part_lo = UFIELD(part_off), part_hi = __shfl_sync(0xffffffffu, uw, (int)(offsetof(GemmUnit, part_off) / 4) + 1);
+            const bool reducer = n_split > 1 && ((UFIELD(c_base) >> 24) & 1);     // GemmUnit::reducer is the 4th byte of that word
+#undef UFIELD
+            const int ext_m = min(BM, M - m0), ext_n = min(BN, N - n0);
+            const int rot = ((m0 >> 6) + (n0 >> 6)) & (CWARPS - 1);     // the same for every K slice of a tile
+            const GemmItem *uitems = items + item_begin;
+            if (KT == 0) {                           // an output without records: the consumers store zeros
+                const int s = acquire();
+                StageHdr *h = hdrs + s;
+                if (lane == 0) { h->flags = F_FIRST | F_LAST; h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                if (lane < UNIT_WORDS) h->u[lane] = uw;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(bars + s));
+                g++;
+                continue;
+            }
+            Producer pr{};
+            begin_item(pr, uitems + p_item, s_base, m0, n0, k00, lane, ctrl, err);
+            for (int t = 0; t < KT; t++) {
+                const int s = acquire();
+                StageHdr *h = hdrs + s;
+                const bool last = (t == KT - 1) && !reducer;
+                if (lane == 0) { h->flags = F_DATA | (t == 0 ? F_FIRST : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                if (last && lane < UNIT_WORDS) h->u[lane] = uw;
+                __syncwarp();
+                if (lane == 0) {
+                    const unsigned sP = smem_u32(stage_base + (size_t)s * STAGE_DOUBLES), bar = smem_u32(bars + s);
+                    mbar_arrive_expect_tx(bar, STAGE_DOUBLES * 8);
+                    bulk_g2s(sP, pr.pP, IMG * 8, bar);
+                    bulk_g2s(sP + IMG * 8, pr.pQ, IMG * 8, bar);
+                }
+                pr.pP += IMG; pr.pQ += IMG; pr.k0 += BK;
+                g++;
+                if (pr.k0 >= pr.K && t + 1 < KT) {
+                    p_item++;
+                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, m0, n0, 0, lane, ctrl, err);
+                }
+            }
+            if (reducer) {
+                // split K, designated reducer (the slice of the tile that comes last in ticket order): once the other
+                // n_split - 1 slices have parked their partial tiles (one arrival per consumer warp each), stream them
+                // through the ring -- 32 KB per slice = two stages -- and let the consumers add them to their registers IN
+                // SLICE ORDER (fixed at plan time: bitwise independent of timing, A22/A23).  The wait is on smaller tickets only.
+                if (lane == 0) {
+                    int *c = counters + tile_id;
+                    const int need = CWARPS * (n_split - 1);
+                    long long spins = 0;
+                    while (ld_acquire(c) < need) {
+                        __nanosleep(32);
+                        if (++spins > (1ll << 26)) { atomicExch(err, 1); break; }
+                    }
+                    *c = 0;                          // self-cleaning for the next launch (this unit is the only reader)
+                }
+                __syncwarp();
+                fence_proxy_async();
+                const double *part = s_base[BASE_PART] + (((long long)part_hi << 32) | (unsigned)part_lo);
+                const int n_red = 2 * (n_split - 1);
+                int r = 0;
+                for (int sl = 0; sl < n_split; sl++) {
+                    if (sl == split_idx) continue;
+                    for (int hh = 0; hh < 2; hh++, r++) {
+                        const int s = acquire();
+                        StageHdr *h = hdrs + s;
+                        const bool last = (r == n_red - 1);
+                        if (lane == 0) { h->flags = F_REDUCE | (hh ? F_HALF : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                        if (last && lane < UNIT_WORDS) h->u[lane] = uw;
+                        __syncwarp();
+                        if (lane == 0) {
+                            const unsigned bar = smem_u32(bars + s);
+                            mbar_arrive_expect_tx(bar, STAGE_DOUBLES * 8);
+                            bulk_g2s(smem_u32(stage_base + (size_t)s * STAGE_DOUBLES), part + (long long)sl * (BM * BN) + hh * STAGE_DOUBLES,
+                                     STAGE_DOUBLES * 8, bar);
                         }
+                        g++;
                     }
                 }
             }
         }
-    }
-    cp_async_wait<0>();
-    if (trace && tid == 0) t_main = globaltimer();
+        {   // no more tickets: tell the consumers to leave
+            const int s = acquire();
+            if (lane == 0) hdrs[s].flags = F_EXIT;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(bars + s));
+        }
+        if (pf.base) {
+            // side job while the launch drains (the ticket queue is empty, HBM is idle): L2 prefetch of this CTA's slice
+            // of the rows the next kernel streams first; fire and forget, 128-byte lines
+            const long long lines = (pf.rows + 15) >> 4;
+            const long long l0 = lines * blockIdx.x / gridDim.x, l1 = lines * (blockIdx.x + 1) / gridDim.x;
+            for (int c = 0; c < pf.cols; c++) {
+                const double *col = pf.base + (long long)c * pf.ld;
+                for (long long l = l0 + lane; l < l1; l += 32)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(col + (l << 4)));
+            }
+        }
+    } else {
+        // ================================================= consumers
+        // Warp -> sub-tile: sub = (warp + rot) mod CWARPS, rows wm = 32 (sub mod 2), columns wn = (sub / 2) * 8 NJW.  The
+        // rotation changes from tile to tile so that the light warps of edge tiles (fewer rows / columns with data) do not
+        // always land on the same SM sub-partition: each sub-partition has its own DMMA pipe, and a CTA advances at the pace
+        // of its busiest warp.
+        const int gq = lane >> 2, tg = lane & 3;
+        int offA[4], offB[NJW];                    // this lane's swizzled offsets for wm = wn = 0 (add wm * BK / wn)
+#pragma unroll
+        for (int k4 = 0; k4 < 4; k4++) offA[k4] = gq * BK + ((((2 * k4 + (tg >> 1)) ^ (2 * (gq & 3)))) << 1) + (tg & 1);
+#pragma unroll
+        for (int j = 0; j < NJW; j++) offB[j] = tg * BN + (((4 * j + (gq >> 1)) ^ (2 * tg)) << 1) + (gq & 1);
 
-    bool writes_c = true;
-    if (u.n_split > 1) {
-        // split K: park the partial tile (fragment order: [slice][register pair][thread], coalesced 16-byte
-        // stores); the last unit of the tile to arrive sums all slices IN SLICE ORDER (bitwise independent of
-        // who is last, A22/A23) with the same thread <-> fragment mapping and writes C from registers.
-        double2 *part = reinterpret_cast<double2 *>(s_base[BASE_PART] + u.part_off);
-        double2 *mine = part + (long long)u.split_idx * (BM * BN / 2);
+        double acc[4][NJW][2];
 #pragma unroll
         for (int i = 0; i < 4; i++)
 #pragma unroll
-            for (int j = 0; j < 4; j++)
-                __stcg(mine + (i * 4 + j) * THREADS + tid, make_double2(acc[i][j][0], acc[i][j][1]));
-        __threadfence();
-        __syncthreads();
-        if (tid == 0) {
-            const int old = atomicAdd(&counters[u.tile_id], 1);
-            s_is_last = (old == u.n_split - 1);
-            if (s_is_last) counters[u.tile_id] = 0;   // self-cleaning for the next launch
-        }
-        __syncthreads();
-        writes_c = s_is_last != 0;
-        if (writes_c) {
-            __threadfence();
-#pragma unroll
-            for (int i = 0; i < 4; i++)
-#pragma unroll
-                for (int j = 0; j < 4; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
-            for (int sl = 0; sl < u.n_split; sl++) {
-                const double2 *src = part + (long long)sl * (BM * BN / 2) + tid;
-#pragma unroll
-                for (int h = 0; h < 2; h++) {          // 8 independent 16-byte loads in flight, twice
-                    double2 v[8];
-#pragma unroll
-                    for (int q = 0; q < 8; q++) v[q] = __ldcg(src + (h * 8 + q) * THREADS);
-#pragma unroll
-                    for (int q = 0; q < 8; q++) {
-                        acc[(h * 8 + q) >> 2][(h * 8 + q) & 3][0] += v[q].x;
-                        acc[(h * 8 + q) >> 2][(h * 8 + q) & 3][1] += v[q].y;
-                    }
-                }
+            for (int j = 0; j < NJW; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+        unsigned long long t_start = 0, t_main = 0;
+
+        // Deferred publish: a finished tile (a T-block tile, or a parked split-K partial) is announced by this WARP on its
+        // own -- fence, then one atomic per warp; the counters count warps -- and not right after its stores, when the fence
+        // would wait for them to drain, but PUBLISH_DELAY stages into the next unit, or as soon as the warp would block.
+        int *pending = nullptr; int pending_g = 0;
+        auto flush = [&]() {
+            if (pending) {
+                fence_proxy_async();      // readers pull these bytes with the TMA unit (async proxy)
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) atomicAdd(pending, 1);
+                pending = nullptr;
             }
-        }
-    }
-    if (writes_c) {
-        double *C = s_base[u.c_base] + u.c_off;
-        const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
-#pragma unroll
-        for (int i = 0; i < 4; i++) {
-            const int row = u.m0 + wm + i * 8 + g;
-            if (row >= u.M) continue;
-#pragma unroll
-            for (int j = 0; j < 4; j++) {
-                const int col = u.n0 + wn + j * 8 + 2 * tg;
-                double *dst = C + (long long)row * u.ldc + col;
-                if (cvec && col + 1 < u.N) {
-                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[i][j][0], acc[i][j][1]);
+        };
+        for (int g = 0;; g++) {
+            const int s = g % STAGES;
+            if (pending && (g - pending_g >= PUBLISH_DELAY || !mbar_test(smem_u32(bars + s), (g / STAGES) & 1))) flush();
+            mbar_wait(smem_u32(bars + s), (g / STAGES) & 1);
+            const StageHdr *h = hdrs + s;
+            const int flags = h->flags;
+            if (flags & F_EXIT) break;
+            if (trace && tid == 0 && (flags & F_FIRST)) t_start = globaltimer();
+            const int sub = (warp + h->rot) & (CWARPS - 1);
+            const int wm = (sub & 1) * 32, wn = (sub >> 1) * (8 * NJW);
+            if (flags & F_DATA) {
+                // sub-tiles of this warp that hold real rows / columns (8-granular): a warp whose data fits in its first
+                // 2 sub-tile rows / columns runs a smaller DMMA block (compile-time bounds), an empty warp tile runs nothing
+                const int mi = min(max(h->ext_m - wm + 7, 0) >> 3, 4);
+                const int nj = min(max(h->ext_n - wn + 7, 0) >> 3, NJW);
+                const double *sP = stage_base + (size_t)s * STAGE_DOUBLES + wm * BK;
+                const double *sQ = stage_base + (size_t)s * STAGE_DOUBLES + IMG + wn;
+                if (NJW == 4) {
+                    if (mi > 2 && nj > 2) mma_ktile<4, NJW>(acc, sP, sQ, offA, offB);
+                    else if (mi > 2 && nj > 0) mma_ktile<4, NJW / 2>(acc, sP, sQ, offA, offB);
+                    else if (mi > 0 && nj > 2) mma_ktile<2, NJW>(acc, sP, sQ, offA, offB);
+                    else if (mi > 0 && nj > 0) mma_ktile<2, NJW / 2>(acc, sP, sQ, offA, offB);
                 } else {
-                    if (col < u.N) dst[0] = acc[i][j][0];
-                    if (col + 1 < u.N) dst[1] = acc[i][j][1];
+                    if (mi > 2 && nj > 1) mma_ktile<4, NJW>(acc, sP, sQ, offA, offB);
+                    else if (mi > 2 && nj > 0) mma_ktile<4, NJW / 2>(acc, sP, sQ, offA, offB);
+                    else if (mi > 0 && nj > 1) mma_ktile<2, NJW>(acc, sP, sQ, offA, offB);
+                    else if (mi > 0 && nj > 0) mma_ktile<2, NJW / 2>(acc, sP, sQ, offA, offB);
+                }
+            } else if (flags & F_REDUCE) {
+                // half of another slice's partial tile, in fragment order [register pair][thread]: add it in place
+                const double2 *src = reinterpret_cast<const double2 *>(stage_base + (size_t)s * STAGE_DOUBLES) + tid;
+                if (flags & F_HALF) {
+#pragma unroll
+                    for (int q = 0; q < 2 * NJW; q++) { const double2 v = src[q * CONSUMERS]; acc[2 + q / NJW][q % NJW][0] += v.x; acc[2 + q / NJW][q % NJW][1] += v.y; }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 2 * NJW; q++) { const double2 v = src[q * CONSUMERS]; acc[q / NJW][q % NJW][0] += v.x; acc[q / NJW][q % NJW][1] += v.y; }
                 }
             }
+            if (flags & F_LAST) {
+                const GemmUnit &u = *reinterpret_cast<const GemmUnit *>(h->u);
+                if (trace && tid == 0) t_main = globaltimer();
+                flush();
+                const bool writes_c = !(u.n_split > 1 && !u.reducer);
+                if (!writes_c) {
+                    // split K, not the reducer: park the partial tile (fragment order: [slice][register pair][thread], coalesced
+                    // 16-byte stores) for the tile's designated reducer
+                    double2 *mine = reinterpret_cast<double2 *>(s_base[BASE_PART] + u.part_off) + (long long)u.split_idx * (BM * BN / 2);
+#pragma unroll
+                    for (int i = 0; i < 4; i++)
+#pragma unroll
+                        for (int j = 0; j < NJW; j++)
+                            __stcg(mine + (i * NJW + j) * CONSUMERS + tid, make_double2(acc[i][j][0], acc[i][j][1]));
+                    pending = counters + u.tile_id; pending_g = g;
+                } else {
+                    double *C = s_base[u.c_base] + u.c_off;
+                    if (u.c_kind == C_ROWMAJOR) {
+                        const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
+#pragma unroll
+                        for (int i = 0; i < 4; i++) {
+                            const int row = u.m0 + wm + i * 8 + gq;
+                            if (row >= u.M) continue;
+#pragma unroll
+                            for (int j = 0; j < NJW; j++) {
+                                const int col = u.n0 + wn + j * 8 + 2 * tg;
+                                double *dst = C + (long long)row * u.ldc + col;
+                                if (cvec && col + 1 < u.N) {
+                                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[i][j][0], acc[i][j][1]);
+                                } else {
+                                    if (col < u.N) dst[0] = acc[i][j][0];
+                                    if (col + 1 < u.N) dst[1] = acc[i][j][1];
+                                }
+                            }
+                        }
+                    } else if (u.c_kind == C_IMG_P) {
+                        // T (M x N) becomes the P operand of stage 2 (K = N): P images [m-tile][k-tile]; the column pair of an
+                        // accumulator is one 16-byte chunk (the pad column of an odd N receives the exact zero it computed)
+                        const int CT = (u.N + BK - 1) / BK;
+                        double *base = C + (long long)(u.m0 / BM) * CT * IMG;
+#pragma unroll
+                        for (int i = 0; i < 4; i++) {
+                            const int r = wm + i * 8 + gq;
+                            if (u.m0 + r >= u.M) continue;
+#pragma unroll
+                            for (int j = 0; j < NJW; j++) {
+                                const int col = u.n0 + wn + j * 8 + 2 * tg;
+                                if (col < u.N)
+                                    *reinterpret_cast<double2 *>(base + (long long)(col / BK) * IMG + img_p_index(r, col % BK)) =
+                                        make_double2(acc[i][j][0], acc[i][j][1]);
+                            }
+                        }
+                    } else {
+                        // T (M x N) becomes the Q operand of stage 2 (K = M): Q images [n-tile][k-tile]
+                        const int CT = (u.M + BK - 1) / BK;
+                        double *base = C + (long long)(u.n0 / BN) * CT * IMG;
+#pragma unroll
+                        for (int i = 0; i < 4; i++) {
+                            const int row = u.m0 + wm + i * 8 + gq;
+                            if (row >= u.M) continue;
+#pragma unroll
+                            for (int j = 0; j < NJW; j++) {
+                                const int c = wn + j * 8 + 2 * tg;
+                                if (u.n0 + c < u.N)
+                                    *reinterpret_cast<double2 *>(base + (long long)(row / BK) * IMG + img_q_index(row % BK, c)) =
+                                        make_double2(acc[i][j][0], acc[i][j][1]);
+                            }
+                        }
+                    }
+                    // this tile of a T block is complete: to be published (release: this warp's stores, then its count)
+                    if (u.signal >= 0) { pending = ctrl + CTRL_DEP0 + u.signal; pending_g = g; }
+                }
+                if (trace && tid == 0) {
+                    unsigned long long *tr = trace + 4ull * h->ticket;
+                    tr[0] = t_start; tr[1] = t_main; tr[2] = globaltimer();
+                    // bits 0-15 SM id, 16-31 k-tiles of the unit, 32-47 CTA, 48 stage-1 unit, 49 split-K unit, 50 wrote C
+                    tr[3] = smid() | ((unsigned long long)u.kt_count << 16) | ((unsigned long long)blockIdx.x << 32) |
+                            ((unsigned long long)(u.signal >= 0) << 48) | ((unsigned long long)(u.n_split > 1) << 49) |
+                            ((unsigned long long)writes_c << 50);
+                }
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+#pragma unroll
+                    for (int j = 0; j < NJW; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(bars + STAGES + s));     // this warp is done with the stage
         }
+        flush();
     }
-    if (pf.base && ticket >= pf.first_ticket) {
-        // side job of the last CTAs in ticket order (done when their unit is done: the launch is draining): L2 prefetch of one slice
-        // of the rows the next kernel streams first; fire and forget, 128-byte lines
-        const long long lines = (pf.rows + 15) >> 4;
-        const int slice = ticket - pf.first_ticket;
-        const long long l0 = lines * slice / pf.n_ctas, l1 = lines * (slice + 1) / pf.n_ctas;
-        for (int c = 0; c < pf.cols; c++) {
-            const double *col = pf.base + (long long)c * pf.ld;
-            for (long long l = l0 + tid; l < l1; l += THREADS)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(col + (l << 4)));
-        }
-    }
-    // publish: this tile of a T block is complete (release: every thread's stores, then the counter);
-    // units that publish nothing skip the fence
-    if (writes_c && u.signal >= 0) __threadfence();
+    // every unit this CTA took is finished; the last CTA to get here resets the control words for the next launch
     __syncthreads();
+    if (ctr && tid == 0) ctr[3] = globaltimer();
     if (tid == 0) {
-        if (writes_c && u.signal >= 0) atomicAdd(&ctrl[CTRL_DEP0 + u.signal], 1);
-        if (trace) {
-            unsigned long long *tr = trace + 4ull * ticket;
-            tr[0] = t_start; tr[1] = t_main; tr[2] = globaltimer(); tr[3] = smid();
-        }
+        __threadfence();
         const int fin = atomicAdd(&ctrl[CTRL_FINISHED], 1);
-        s_is_last = (fin == n_units - 1);
+        s_is_last = (fin == (int)gridDim.x - 1);
     }
     __syncthreads();
-    if (s_is_last) {   // every other unit has finished: reset the control words for the next launch
+    if (s_is_last) {
         for (int e = tid; e < CTRL_DEP0 + n_deps; e += THREADS) ctrl[e] = 0;
     }
 }
@@ -387,16 +546,22 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 }  // namespace
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
-typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int, int,
-                        unsigned long long *, Prefetch);
-struct Variant { const char *name; gemm_fn fn; int smem; };
+typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int,
+                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long);
+struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
-    {"s3b4m2", grouped_gemm_kernel<3, 4, 2>, smem_bytes(3)},   // default: measured best at cfg3 / 5a / 5b / 4096 sweep
-    {"s3b4m0", grouped_gemm_kernel<3, 4, 0>, smem_bytes(3)},
-    {"s3b4m1", grouped_gemm_kernel<3, 4, 1>, smem_bytes(3)},
-    {"s4b3m2", grouped_gemm_kernel<4, 3, 2>, smem_bytes(4)},
+#if DMRG_CWARPS == 8
+    {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},
+    {"s4b3", grouped_gemm_kernel<4, 3>, smem_bytes(4), 3},
+    {"s5b2", grouped_gemm_kernel<5, 2>, smem_bytes(5), 2},
+#else
+    {"s4b3", grouped_gemm_kernel<4, 3>, smem_bytes(4), 3},
+    {"s3b4", grouped_gemm_kernel<3, 4>, smem_bytes(3), 4},
+    {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},
+#endif
 };
 static const Variant *g_variant = &kVariants[0];
+static int g_ctas_per_sm = 0;
 
 cudaError_t gemm_kernel_setup() {
     if (const char *e = getenv("DMRG_GEMM_VARIANT"))
@@ -406,12 +571,18 @@ cudaError_t gemm_kernel_setup() {
         cudaError_t err = cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem);
         if (err != cudaSuccess) return err;
     }
+    int occ = 0;
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, g_variant->fn, THREADS, g_variant->smem);
+    if (err != cudaSuccess) return err;
+    g_ctas_per_sm = std::max(1, std::min(occ, g_variant->ctas_per_sm));
+    if (const char *e = getenv("DMRG_CTAS_PER_SM")) g_ctas_per_sm = std::max(1, std::min(g_ctas_per_sm, atoi(e)));
     return cudaSuccess;
 }
 
 int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in) {
     BasePtrs b;
-    b.p[BASE_X] = const_cast<double *>(x);
+    b.p[BASE_XP] = p->ximg_p;
+    b.p[BASE_XQ] = p->ximg_q;
     b.p[BASE_Y] = y;
     b.p[BASE_T] = p->tws;
     b.p[BASE_POOL] = p->pool;
@@ -421,16 +592,13 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
     const int n_units = p->n_units1 + p->n_units2;
     p->launches += n_units > 0 ? 1 : 0;
     if (n_units > 0) {
-        const int xvec = ((reinterpret_cast<uintptr_t>(x) & 15) == 0) ? 1 : 0;
         const int yvec = ((reinterpret_cast<uintptr_t>(y) & 15) == 0) ? 1 : 0;
         Prefetch pf;
-        if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) {
-            pf = *pf_in;
-            pf.n_ctas = std::min(n_units, 4 * p->sm_count);
-            pf.first_ticket = n_units - pf.n_ctas;
-        }
-        g_variant->fn<<<n_units, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
-                                                                 p->n_deps, done_flag, xvec, yvec, p->trace, pf);
+        if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) pf = *pf_in;
+        const int grid = std::min(n_units, g_ctas_per_sm * p->sm_count);     // persistent: one wave, units by ticket
+        g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
+                                                              p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
+                                                              p->xsegs, p->n_xsegs, x, p->n);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

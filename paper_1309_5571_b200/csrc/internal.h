@@ -13,16 +13,29 @@ namespace dmrg {
 // Every product on the path is brought to the form  C(MxN) = sum_items P(MxK) * Q(KxN), all
 // row-major: right-block factors are stored transposed (B^T) and left-block factors pre-scaled
 // by the record coefficient at plan time (operators are constant over the iteration, L340).
-enum Base : uint8_t { BASE_X = 0, BASE_Y = 1, BASE_T = 2, BASE_POOL = 3, BASE_PART = 4, BASE_COUNT = 5 };
+enum Base : uint8_t { BASE_XP = 0, BASE_Y = 1, BASE_T = 2, BASE_POOL = 3, BASE_PART = 4, BASE_XQ = 5, BASE_COUNT = 6 };
 
+// Operand storage.  Every operand of the grouped kernel is stored as TILE IMAGES: 8 KB blocks holding exactly what one
+// k-tile of the kernel keeps in shared memory, XOR-swizzled so that the DMMA fragment loads are bank-conflict free, edges
+// zero-padded.  One k-tile of an operand = one bulk copy (cp.async.bulk).
+//   P operand (M x K): image [m-tile][k-tile] at  off + (mt * ceil(K/16) + kt) * IMG, element (r, c) of the 64 x 16 tile
+//                      at img_p_index(r, c);
+//   Q operand (K x N): image [n-tile][k-tile] at  off + (nt * ceil(K/16) + kt) * IMG, element (k, c) of the 16 x 64 tile
+//                      at img_q_index(k, c).
+// BASE_POOL: the repacked operators (written once per plan); BASE_T: the T blocks between the two GEMM stages (written by
+// the stage-1 epilogues); BASE_XP / BASE_XQ: the input vector's segments as P images (X_ik as M x K = d_i x d_k) and as
+// Q images (K x N = d_i x d_k), written by phase 0 of every apply (all CTAs) from the caller's row-major vector.
 struct GemmItem {
-    long long p_off, q_off;   // element offsets in their bases
-    int ldp, ldq, K;
+    long long p_off, q_off;   // element offsets of the operands' first images in their bases
+    int K;
     uint8_t p_base, q_base;
-    uint8_t p_vec2, q_vec2;   // 16-byte loads legal (even offset, even ld)
+    uint8_t pad[2];
     int dep;                  // index of the T-block ready counter this item waits on (-1: reads no T)
-    int dep_need;             // tiles of that T block: the counter value that means "complete"
+    int dep_need;             // 4 x tiles of that T block (one count per consumer warp): the counter value that means "complete"
 };
+
+// Phase 0 table, one entry per segment X_ik (d_i x d_k, row-major at x + seg_off, ascending seg_off): where its P and Q images start
+struct XSeg { long long seg_off, xp_off, xq_off; int di, dk; };
 
 struct GemmUnit {
     long long c_off;          // C(0,0) in its base
@@ -34,32 +47,46 @@ struct GemmUnit {
     int tile_id;              // split-K counter index (-1: not split)
     int split_idx, n_split;
     uint8_t c_base, c_vec2;
-    uint8_t pad[2];
+    uint8_t c_kind;           // C_ROWMAJOR (caller vector) | C_IMG_P | C_IMG_Q (T block, stored as the images stage 2 loads)
+    uint8_t reducer;          // split-K: this slice (the tile's last in ticket order) sums the parked partials and writes C
     int signal;               // T-block ready counter to bump once this tile of T is written (-1: none)
     int cost;                 // scheduling weight (DMMA count + per-k-tile overhead)
     int item0, k00;           // where kt_begin falls: item index inside the unit's item list and k offset inside that item
 };
 
-// control words of one apply (device ints): ticket dispenser, finished count, then one ready counter per T block
-enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_DEP0 = 2 };
+// control words of one apply (device ints): ticket dispenser, finished count, X-image count, then one ready counter per T block
+enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_XREADY = 2, CTRL_DEP0 = 3 };   // XREADY: CTAs whose share of the X images is written
 
 struct BasePtrs { double *p[BASE_COUNT]; };
 
 // tile shape of the grouped kernel (gemm.cu is compiled for exactly these)
 constexpr int BM = 64, BN = 64, BK = 16;
+constexpr int IMG = BM * BK;    // doubles per tile image (P: 64 x 16, Q: 16 x 64)
+#ifndef DMRG_CWARPS
+#define DMRG_CWARPS 8
+#endif
+constexpr int CWARPS = DMRG_CWARPS;   // consumer warps per CTA of the grouped kernel; the ready counters count warps
+enum CKind : uint8_t { C_ROWMAJOR = 0, C_IMG_P = 1, C_IMG_Q = 2 };
+// 16-byte chunks of a row are XOR-ed with 2 * (row % 4): the 8 rows x 4 k (P) / 4 k x 8 columns (Q) of a DMMA fragment
+// then fall on 32 distinct banks per half-warp.
+__host__ __device__ inline int img_p_index(int r, int c) { return r * BK + ((((c >> 1) ^ (2 * (r & 3)))) << 1) + (c & 1); }
+__host__ __device__ inline int img_q_index(int k, int c) { return k * BN + ((((c >> 1) ^ (2 * (k & 3)))) << 1) + (c & 1); }
+inline long long img_p_elems(long long M, long long K) { return ((M + BM - 1) / BM) * ((K + BK - 1) / BK) * IMG; }
+inline long long img_q_elems(long long K, long long N) { return ((N + BN - 1) / BN) * ((K + BK - 1) / BK) * IMG; }
 
 // ---- plan-time device jobs ----
-struct RepackJob {            // dst(rows x cols, ld) = s1*op(src1) + s2*op(src2), op = transpose if flag
+struct RepackJob {            // dst(rows x cols) = s1*op(src1) + s2*op(src2), op = transpose if flag; dst stored as images
     const double *src1, *src2;
     long long dst_off;
-    int ld1, ld2, ldd, rows, cols;   // rows/cols of dst
+    int ld1, ld2, rows, cols;        // rows/cols of dst
     int transpose;
+    int q_role;                      // 0: P images (rows = M, cols = K); 1: Q images (rows = K, cols = N)
     double s1, s2;
 };
-struct DiagJob {              // D_seg[a,b] += c * da[a] * db[b]; null pointer = all ones
+struct DiagJob {              // D_seg[a,b] += c * A(a,a) * B(b,b); null pointer = all ones
     long long seg_off;
-    const double *da, *db;    // first diagonal element
-    long long stride_a, stride_b;    // ld+1
+    const double *da, *db;    // first image of the left (P role) / right (Q role) factor
+    int ka, kb;               // their K (P: columns, Q: rows) -- fixes the image grid
     int rows, cols;
     double c;
 };
@@ -78,7 +105,8 @@ struct DavState {
     int k_used;               // basis size in the last executed step
     int sweeps;               // Jacobi sweeps of the last small eig
     int e_k;                  // size of the B whose eigenvectors E holds (0 = invalid)
-    int pad[2];
+    int gemm_error;           // sticky: a dependency wait of the grouped kernel gave up (lost / interleaved launch)
+    int pad[1];
 };
 
 struct Timing { bool enabled = false; cudaEvent_t ev[10]; double ms[8]; bool created = false; };
@@ -95,6 +123,8 @@ struct Plan {
     std::vector<long long> segOff;
     // device memory
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
+    double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
+    XSeg *xsegs = nullptr; int n_xsegs = 0;
     int *counters = nullptr;
     GemmItem *items = nullptr;          // stage-1 items, then stage-2 items
     GemmUnit *units = nullptr;          // ticket order: stage-1 units, then stage-2 units

@@ -32,13 +32,19 @@ __global__ void repack_kernel(RepackJob j, double *pool) {
     __shared__ double tile[32][33];
     double *dst = pool + j.dst_off;
     const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    // image address of element (r, c) of the repacked matrix (internal.h: P images [m-tile][k-tile], Q images [n-tile][k-tile])
+    const int KT = j.q_role ? (j.rows + BK - 1) / BK : (j.cols + BK - 1) / BK;
+    auto at = [&](int r, int c) -> double & {
+        if (j.q_role) return dst[((long long)(c / BN) * KT + r / BK) * IMG + img_q_index(r % BK, c % BN)];
+        return dst[((long long)(r / BM) * KT + c / BK) * IMG + img_p_index(r % BM, c % BK)];
+    };
     if (!j.transpose) {
         for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
             int r = r0 + rr, c = c0 + threadIdx.x;
             if (r < j.rows && c < j.cols) {
                 double v = j.s1 * j.src1[(long long)r * j.ld1 + c];
                 if (j.src2) v += j.s2 * j.src2[(long long)r * j.ld2 + c];
-                dst[(long long)r * j.ldd + c] = v;
+                at(r, c) = v;
             }
         }
     } else {
@@ -55,7 +61,7 @@ __global__ void repack_kernel(RepackJob j, double *pool) {
         __syncthreads();
         for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
             int r = r0 + rr, c = c0 + threadIdx.x;
-            if (r < j.rows && c < j.cols) dst[(long long)r * j.ldd + c] = tile[threadIdx.x][rr];
+            if (r < j.rows && c < j.cols) at(r, c) = tile[threadIdx.x][rr];
         }
     }
 }
@@ -65,21 +71,21 @@ __global__ void diag_kernel(DiagJob j, double *D) {
     long long tot = (long long)j.rows * j.cols;
     if (idx >= tot) return;
     int a = (int)(idx / j.cols), b = (int)(idx % j.cols);
-    double va = j.da ? j.da[a * j.stride_a] : 1.0;
-    double vb = j.db ? j.db[b * j.stride_b] : 1.0;
+    // diagonal elements out of the tile images: A is a P operand (rows x ka), B^T a Q operand (kb x cols)
+    double va = j.da ? j.da[((long long)(a / BM) * ((j.ka + BK - 1) / BK) + a / BK) * IMG + img_p_index(a % BM, a % BK)] : 1.0;
+    double vb = j.db ? j.db[((long long)(b / BN) * ((j.kb + BK - 1) / BK) + b / BK) * IMG + img_q_index(b % BK, b % BN)] : 1.0;
     D[j.seg_off + idx] += j.c * (va * vb);
 }
 
 // ---------------------------------------------------------------- host helpers
 namespace {
 
-struct PoolEntry { long long off; int rows, cols, ld; };
+struct PoolEntry { long long off; int rows, cols; bool q_role; };
 struct FactorBlk { int src, dst, entry; };          // entry = pool index
 struct Term { bool A_id, B_id; std::vector<FactorBlk> A, B; };
 struct Record { int A, B, in_pair, out_pair; };      // pool entries or -1 (identity)
-struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; int out_pair; };
+struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; int out_pair; uint8_t c_kind; };
 
-inline long long round_up(long long v, long long a) { return (v + a - 1) / a * a; }
 
 struct Builder {
     Plan *p;
@@ -89,22 +95,24 @@ struct Builder {
     long long pool_elems = 0;
     long long op_elems = 0;
 
-    int add_entry(const dmrg_block_op &op, int b, const std::vector<int> &dims, bool transpose, double scale,
+    // q_role: the entry is a right-block factor, stored as B^T = the Q operand (K x N) of its products; left-block
+    // factors are P operands (M x K).  Either way the entry is a grid of zero-padded 8 KB tile images.
+    int add_entry(bool q_role, const dmrg_block_op &op, int b, const std::vector<int> &dims, bool transpose, double scale,
                   const dmrg_block_op *op2 = nullptr, int b2 = -1, double scale2 = 0.0) {
         int rs = dims[op.dst[b]], cs = dims[op.src[b]];   // source block shape rs x cs
         PoolEntry e;
         e.rows = transpose ? cs : rs;
         e.cols = transpose ? rs : cs;
-        e.ld = (int)round_up(std::max(e.cols, 1), 2);
+        e.q_role = q_role;
         e.off = pool_elems;
-        pool_elems += round_up((long long)std::max(e.rows, 1) * e.ld, 16);
+        pool_elems += q_role ? img_q_elems(e.rows, e.cols) : img_p_elems(e.rows, e.cols);
         op_elems += (long long)e.rows * e.cols;
         RepackJob j{};
         j.src1 = op.data + op.offset[b];
         j.ld1 = op.ld[b];
         j.s1 = scale;
         if (op2) { j.src2 = op2->data + op2->offset[b2]; j.ld2 = op2->ld[b2]; j.s2 = scale2; }
-        j.dst_off = e.off; j.ldd = e.ld; j.rows = e.rows; j.cols = e.cols; j.transpose = transpose ? 1 : 0;
+        j.dst_off = e.off; j.rows = e.rows; j.cols = e.cols; j.transpose = transpose ? 1 : 0; j.q_role = q_role ? 1 : 0;
         jobs.push_back(j);
         pool.push_back(e);
         return (int)pool.size() - 1;
@@ -256,11 +264,11 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                 int e = -1;
                 const bool tr = side == 1;   // right factors are stored as B^T
                 if (!hs[s].empty() && useD && !ds[s].empty())
-                    e = bl.add_entry(H, hs[s][0], dims, tr, 1.0, &Dd, ds[s][0], pr->U);
+                    e = bl.add_entry(tr, H, hs[s][0], dims, tr, 1.0, &Dd, ds[s][0], pr->U);
                 else if (!hs[s].empty())
-                    e = bl.add_entry(H, hs[s][0], dims, tr, 1.0);
+                    e = bl.add_entry(tr, H, hs[s][0], dims, tr, 1.0);
                 else if (useD && !ds[s].empty())
-                    e = bl.add_entry(Dd, ds[s][0], dims, tr, pr->U);
+                    e = bl.add_entry(tr, Dd, ds[s][0], dims, tr, pr->U);
                 if (e >= 0) (side == 0 ? t.A : t.B).push_back({s, s, e});
             }
             terms.push_back(std::move(t));
@@ -279,15 +287,15 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
             for (int b = 0; b < pr->Sp_L.n_blocks; b++) {
                 int s = pr->Sp_L.src[b], d = pr->Sp_L.dst[b];
                 if (!p->dimL[s] || !p->dimL[d]) continue;
-                tp.A.push_back({s, d, bl.add_entry(pr->Sp_L, b, p->dimL, false, half)});
-                tm.A.push_back({d, s, bl.add_entry(pr->Sp_L, b, p->dimL, true, half)});
+                tp.A.push_back({s, d, bl.add_entry(false, pr->Sp_L, b, p->dimL, false, half)});
+                tm.A.push_back({d, s, bl.add_entry(false, pr->Sp_L, b, p->dimL, true, half)});
             }
             for (int b = 0; b < pr->Sp_R.n_blocks; b++) {
                 int s = pr->Sp_R.src[b], d = pr->Sp_R.dst[b];
                 if (!p->dimR[s] || !p->dimR[d]) continue;
                 // S-_R block d->s has matrix blk^T, so its B^T is blk as stored
-                tp.B.push_back({d, s, bl.add_entry(pr->Sp_R, b, p->dimR, false, 1.0)});
-                tm.B.push_back({s, d, bl.add_entry(pr->Sp_R, b, p->dimR, true, 1.0)});
+                tp.B.push_back({d, s, bl.add_entry(true, pr->Sp_R, b, p->dimR, false, 1.0)});
+                tm.B.push_back({s, d, bl.add_entry(true, pr->Sp_R, b, p->dimR, true, 1.0)});
             }
             terms.push_back(std::move(tp));
             terms.push_back(std::move(tm));
@@ -296,10 +304,10 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
             Term tz; tz.A_id = tz.B_id = false;
             for (int b = 0; b < pr->Sz_L.n_blocks; b++)
                 if (p->dimL[pr->Sz_L.src[b]])
-                    tz.A.push_back({pr->Sz_L.src[b], pr->Sz_L.dst[b], bl.add_entry(pr->Sz_L, b, p->dimL, false, zz)});
+                    tz.A.push_back({pr->Sz_L.src[b], pr->Sz_L.dst[b], bl.add_entry(false, pr->Sz_L, b, p->dimL, false, zz)});
             for (int b = 0; b < pr->Sz_R.n_blocks; b++)
                 if (p->dimR[pr->Sz_R.src[b]])
-                    tz.B.push_back({pr->Sz_R.src[b], pr->Sz_R.dst[b], bl.add_entry(pr->Sz_R, b, p->dimR, true, 1.0)});
+                    tz.B.push_back({pr->Sz_R.src[b], pr->Sz_R.dst[b], bl.add_entry(true, pr->Sz_R, b, p->dimR, true, 1.0)});
             terms.push_back(std::move(tz));
         }
     } else {
@@ -313,14 +321,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                 int s = CL[sg]->src[b], d = CL[sg]->dst[b];
                 if (!p->dimL[s] || !p->dimL[d]) continue;
                 const double c = -pr->t * parity_sign(s);   // s = input of c+, = output of c
-                t1.A.push_back({s, d, bl.add_entry(*CL[sg], b, p->dimL, false, c)});
-                t2.A.push_back({d, s, bl.add_entry(*CL[sg], b, p->dimL, true, c)});
+                t1.A.push_back({s, d, bl.add_entry(false, *CL[sg], b, p->dimL, false, c)});
+                t2.A.push_back({d, s, bl.add_entry(false, *CL[sg], b, p->dimL, true, c)});
             }
             for (int b = 0; b < CR[sg]->n_blocks; b++) {
                 int s = CR[sg]->src[b], d = CR[sg]->dst[b];
                 if (!p->dimR[s] || !p->dimR[d]) continue;
-                t1.B.push_back({d, s, bl.add_entry(*CR[sg], b, p->dimR, false, 1.0)});   // c_R: B^T = blk
-                t2.B.push_back({s, d, bl.add_entry(*CR[sg], b, p->dimR, true, 1.0)});    // c+_R: B^T = blk^T
+                t1.B.push_back({d, s, bl.add_entry(true, *CR[sg], b, p->dimR, false, 1.0)});   // c_R: B^T = blk
+                t2.B.push_back({s, d, bl.add_entry(true, *CR[sg], b, p->dimR, true, 1.0)});    // c+_R: B^T = blk^T
             }
             terms.push_back(std::move(t1));
             terms.push_back(std::move(t2));
@@ -361,20 +369,30 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     long long tws_elems = 0, flops = 0, flops1 = 0;
     int n_gemms = 0;
     auto vec2 = [](long long off, int ld) { return (uint8_t)((off % 2 == 0 && ld % 2 == 0) ? 1 : 0); };
+    // the input vector's segments as tile images (both operand roles), rewritten by phase 0 of every apply
+    std::vector<long long> xpOff(P), xqOff(P);
+    std::vector<XSeg> xsegs;
+    long long xp_elems = 0, xq_elems = 0;
+    for (int op = 0; op < P; op++) {
+        const int di = p->dimL[p->pairL[op]], dk = p->dimR[p->pairR[op]];
+        xpOff[op] = xp_elems; xp_elems += img_p_elems(di, dk);
+        xqOff[op] = xq_elems; xq_elems += img_q_elems(di, dk);
+        xsegs.push_back({p->segOff[op], xpOff[op], xqOff[op], di, dk});
+    }
     for (const Record &r : recs) {
         const int i = p->pairL[r.in_pair], k = p->pairR[r.in_pair];
         const int j = p->pairL[r.out_pair], l = p->pairR[r.out_pair];
         const long long di = p->dimL[i], dk = p->dimR[k], dj = p->dimL[j], dl = p->dimR[l];
-        const long long xoff = p->segOff[r.in_pair];
+        const long long xp = xpOff[r.in_pair], xq = xqOff[r.in_pair];
         GemmItem it2{};
         int dep = -1;             // stage-1 task whose T block this record's stage-2 item reads
         if (r.B < 0) {            // A (x) I :  X'_jk += A X_ik
             const PoolEntry &A = bl.pool[r.A];
-            it2 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
+            it2 = {A.off, xq, (int)di, BASE_POOL, BASE_XQ};
             flops += 2 * dj * di * dk; n_gemms += 1;
         } else if (r.A < 0) {     // I (x) B :  X'_il += X_ik B^T
             const PoolEntry &B = bl.pool[r.B];
-            it2 = {xoff, B.off, (int)dk, B.ld, (int)dk, BASE_X, BASE_POOL, vec2(xoff, (int)dk), vec2(B.off, B.ld)};
+            it2 = {xp, B.off, (int)dk, BASE_XP, BASE_POOL};
             flops += 2 * di * dk * dl; n_gemms += 1;
         } else {
             const PoolEntry &A = bl.pool[r.A], &B = bl.pool[r.B];
@@ -383,19 +401,17 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
             n_gemms += 2;
             GemmItem it1{};
             TaskHost t1{};
-            if (f1 <= f2) {
-                const int ldt = (int)round_up(dl, 2);
-                const long long toff = tws_elems; tws_elems += round_up(di * ldt, 16);
-                it1 = {xoff, B.off, (int)dk, B.ld, (int)dk, BASE_X, BASE_POOL, vec2(xoff, (int)dk), vec2(B.off, B.ld)};
-                t1 = {BASE_T, toff, ldt, (int)di, (int)dl, 0, 1};
-                it2 = {A.off, toff, A.ld, ldt, (int)di, BASE_POOL, BASE_T, vec2(A.off, A.ld), 1};
+            if (f1 <= f2) {       // T (d_i x d_l) is the Q operand of stage 2 (K = d_i): stored as Q images
+                const long long toff = tws_elems; tws_elems += img_q_elems(di, dl);
+                it1 = {xp, B.off, (int)dk, BASE_XP, BASE_POOL};
+                t1 = {BASE_T, toff, 0, (int)di, (int)dl, 0, 1, 0, C_IMG_Q};
+                it2 = {A.off, toff, (int)di, BASE_POOL, BASE_T};
                 flops += f1; flops1 += 2 * di * dk * dl;
-            } else {
-                const int ldt = (int)round_up(dk, 2);
-                const long long toff = tws_elems; tws_elems += round_up(dj * ldt, 16);
-                it1 = {A.off, xoff, A.ld, (int)dk, (int)di, BASE_POOL, BASE_X, vec2(A.off, A.ld), vec2(xoff, (int)dk)};
-                t1 = {BASE_T, toff, ldt, (int)dj, (int)dk, 0, 1};
-                it2 = {toff, B.off, ldt, B.ld, (int)dk, BASE_T, BASE_POOL, 1, vec2(B.off, B.ld)};
+            } else {              // T (d_j x d_k) is the P operand of stage 2 (K = d_k): stored as P images
+                const long long toff = tws_elems; tws_elems += img_p_elems(dj, dk);
+                it1 = {A.off, xq, (int)di, BASE_POOL, BASE_XQ};
+                t1 = {BASE_T, toff, 0, (int)dj, (int)dk, 0, 1, 0, C_IMG_P};
+                it2 = {toff, B.off, (int)dk, BASE_T, BASE_POOL};
                 flops += f2; flops1 += 2 * dj * di * dk;
             }
             t1.item_begin = (int)items1.size();
@@ -406,7 +422,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
             tasks1.push_back(t1);
         }
         it2.dep = dep;
-        it2.dep_need = dep < 0 ? 0 : ((tasks1[dep].M + BM - 1) / BM) * ((tasks1[dep].N + BN - 1) / BN);
+        it2.dep_need = dep < 0 ? 0 : CWARPS * ((tasks1[dep].M + BM - 1) / BM) * ((tasks1[dep].N + BN - 1) / BN);   // one count per consumer warp
         out_items[r.out_pair].push_back(it2);
     }
     // inside one output the records that read X directly come first in the K order, so that a stage-2 unit
@@ -415,7 +431,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return (a.dep < 0) > (b.dep < 0); });
     for (int op = 0; op < P; op++) {
         TaskHost t{};
-        t.c_base = BASE_Y; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
+        t.c_base = BASE_Y; t.c_kind = C_ROWMAJOR; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
         t.M = p->dimL[p->pairL[op]]; t.N = p->dimR[p->pairR[op]];
         t.item_begin = (int)items2.size(); t.item_count = (int)out_items[op].size(); t.out_pair = op;
         for (const GemmItem &it : out_items[op]) items2.push_back(it);
@@ -439,7 +455,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     const int kt_min = 6;
     // target: ~units_per_sm units per SM over the whole apply (DMRG_UNITS_PER_SM overrides for experiments)
     // (measured: 16 is best at cfg 3 / 5a, ~280 k-tile units per SM; 24 at the 4096 sweep, 2200 per SM; flat beyond)
-    long long ups = (Wtot / std::max(p->sm_count, 1) < 1000) ? 16 : 24;
+    long long ups = (Wtot / std::max(p->sm_count, 1) < 1000) ? 12 : 24;   // re-measured with the persistent kernel: 10-12 best at cfg 3 / 5a
     if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
     const long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
     std::vector<long long> out_cost(P, 0);
@@ -486,7 +502,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                     u.item_begin = t.item_begin + item_shift; u.item_count = t.item_count;
                     u.kt_begin = begin; u.kt_count = base + (sp < rem ? 1 : 0); begin += u.kt_count;
                     u.tile_id = tile_id; u.split_idx = sp; u.n_split = ns;
-                    u.c_base = t.c_base; u.c_vec2 = vec2(t.c_off, t.ldc);
+                    u.c_base = t.c_base; u.c_kind = t.c_kind; u.c_vec2 = vec2(t.c_off, t.ldc);
                     u.signal = signals ? (int)ti : -1;
                     u.cost = u.kt_count * (4 * sub + 64);
                     {   // resolve kt_begin to (item, k offset) here, so that the kernel does not walk the item list
@@ -528,6 +544,11 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     order_units(units2, uo2);
     std::vector<GemmUnit> units(units1);
     units.insert(units.end(), units2.begin(), units2.end());
+    {   // split-K: the slice of a tile that comes LAST in ticket order is its reducer (it waits on smaller tickets only)
+        std::vector<int> last_of(n_counters, -1);
+        for (size_t q = 0; q < units.size(); q++) if (units[q].tile_id >= 0) last_of[units[q].tile_id] = (int)q;
+        for (int t = 0; t < n_counters; t++) if (last_of[t] >= 0) units[last_of[t]].reducer = 1;
+    }
     std::vector<GemmItem> items(items1);
     items.insert(items.end(), items2.begin(), items2.end());
     p->n_deps = (int)tasks1.size();
@@ -536,6 +557,13 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
     CUDA_TRY(p, dev_alloc(p, &p->tws, tws_elems));
     CUDA_TRY(p, dev_alloc(p, &p->part, part_elems));
+    CUDA_TRY(p, dev_alloc(p, &p->ximg_p, xp_elems));
+    CUDA_TRY(p, dev_alloc(p, &p->ximg_q, xq_elems));
+    CUDA_TRY(p, cudaMemset(p->ximg_p, 0, sizeof(double) * std::max<long long>(xp_elems, 1)));   // the pads stay zero for good
+    CUDA_TRY(p, cudaMemset(p->ximg_q, 0, sizeof(double) * std::max<long long>(xq_elems, 1)));
+    CUDA_TRY(p, dev_alloc(p, &p->xsegs, (long long)xsegs.size()));
+    if (!xsegs.empty()) CUDA_TRY(p, cudaMemcpy(p->xsegs, xsegs.data(), xsegs.size() * sizeof(XSeg), cudaMemcpyHostToDevice));
+    p->n_xsegs = (int)xsegs.size();
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
@@ -543,7 +571,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + p->n_deps));
     CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + p->n_deps)));
     if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
-        p->trace_units = (int)units.size();
+        // 4 words per unit, then 4 words per CTA (phase stamps: entry, X images written, producer released, exit)
+        p->trace_units = (int)units.size() + 8 * p->sm_count;
         CUDA_TRY(p, dev_alloc(p, &p->trace, 4LL * std::max<long long>(p->trace_units, 1)));
         CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     }
@@ -570,8 +599,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         dj.seg_off = p->segOff[r.in_pair];
         dj.rows = p->dimL[p->pairL[r.in_pair]]; dj.cols = p->dimR[p->pairR[r.in_pair]];
         dj.c = 1.0;   // the coefficient is already folded into the left factor
-        if (r.A >= 0) { dj.da = p->pool + bl.pool[r.A].off; dj.stride_a = bl.pool[r.A].ld + 1; }
-        if (r.B >= 0) { dj.db = p->pool + bl.pool[r.B].off; dj.stride_b = bl.pool[r.B].ld + 1; }
+        if (r.A >= 0) { dj.da = p->pool + bl.pool[r.A].off; dj.ka = bl.pool[r.A].cols; }
+        if (r.B >= 0) { dj.db = p->pool + bl.pool[r.B].off; dj.kb = bl.pool[r.B].rows; }
         long long tot = (long long)dj.rows * dj.cols;
         diag_kernel<<<(unsigned)((tot + 255) / 256), 256>>>(dj, p->D);
     }
@@ -599,7 +628,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     s.flop_per_apply = flops; s.flop_stage1 = flops1; s.flop_stage2 = flops - flops1; s.operator_elems = bl.op_elems; s.apply_bytes = 8 * (bl.op_elems + 2 * p->n);
     s.stage1_units = p->n_units1; s.stage2_units = p->n_units2; s.stage2_split_tiles = split_tiles2;
     s.pool_bytes = 8 * bl.pool_elems;
-    s.workspace_bytes = 8 * (tws_elems + part_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
+    s.workspace_bytes = 8 * (tws_elems + part_elems + xp_elems + xq_elems + 3 * p->n + (long long)p->vec_grid * (KMAX + 2));
     s.device_bytes = p->device_bytes;
     s.kernel_launches_per_apply = 1;
     // apply, V^T w, small eig, residual (+ V^T t fused), { V^T t from the second pass on }, t -= V s, append; +3 on a restart step
@@ -611,6 +640,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
 void plan_free(Plan *p) {
     if (!p) return;
     cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
+    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs);
     cudaFree(p->items); cudaFree(p->units); cudaFree(p->ctrl); cudaFree(p->trace);
     cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
