@@ -15,8 +15,8 @@
 //
 // sm_100a specifics.  FP64 has no tcgen05/TMEM path (ptxas rejects .kind::f64); the FP64 tensor instruction is
 // mma.sync m8n8k4 -> SASS DMMA.8x8x4 (one per 16 clocks per SM sub-partition: 37 TFLOP/s per chip).
-// The kernel is WARP-SPECIALISED and PERSISTENT: each CTA = 4 consumer warps (2x2, warp tile 32x32, register
-// accumulators) + 1 producer warp, 3 CTAs per SM, a ring of STAGES k-tiles (64x16 of P, 16x64 of Q; 16 KB) with one
+// The kernel is WARP-SPECIALISED and PERSISTENT: each CTA = 8 consumer warps (8 of the tile's 64 8x8 accumulator
+// sub-tiles each, in registers) + 1 producer warp, 2 CTAs per SM, a ring of STAGES k-tiles (64x16 of P, 16x64 of Q; 16 KB) with one
 // "full" and one "empty" mbarrier per stage -- there is no CTA-wide barrier in the main loop, and the producer
 // runs ahead across unit boundaries (the next unit's first k-tiles land while the consumers are in the epilogue).
 // Every operand (the repacked operator pool, the T workspace and -- after phase 0 of the kernel, in which all CTAs
@@ -33,10 +33,9 @@ namespace dmrg {
 
 namespace {
 
-constexpr int CONSUMERS = CWARPS * 32;     // consumer warps: 2 (M) x CWARPS/2 (N); warp tile 32 x (128 / CWARPS)
+constexpr int CONSUMERS = CWARPS * 32;     // eight consumer warps, 8 of the tile's 64 accumulator sub-tiles each
 constexpr int THREADS = CONSUMERS + 32;    // + 1 producer warp
-constexpr int NJW = 16 / CWARPS;           // 8-column sub-tiles per warp: 4 (four warps) or 2 (eight warps)
-static_assert(CWARPS == 4 || CWARPS == 8, "consumer layout");
+static_assert(CWARPS == 8, "consumer layouts below are written for eight warps");
 constexpr int STAGE_DOUBLES = 2 * IMG;     // P image + Q image
 constexpr int UNIT_WORDS = (int)(sizeof(GemmUnit) / 4);
 static_assert(UNIT_WORDS <= 32, "one lane per word of the unit descriptor");
@@ -45,7 +44,7 @@ enum : int { F_DATA = 1, F_LAST = 2, F_EXIT = 4, F_FIRST = 8, F_REDUCE = 16, F_H
 constexpr int PUBLISH_DELAY = 2;           // stages a consumer warp works on before it fences and signals a finished tile
 struct StageHdr {
     int flags, ticket, ext_m, ext_n;       // ext: rows / columns of the 64x64 tile that hold data
-    int rot, pad[3];                       // sub-tile rotation of the unit (see the consumers)
+    int rot, layout, pad[2];               // sub-tile rotation and warp layout of the unit (see the consumers)
     int u[UNIT_WORDS];                     // the unit descriptor (valid in the unit's last stage: epilogue)
 };
 constexpr int smem_bytes(int stages) { return stages * (STAGE_DOUBLES * 8 + (int)sizeof(StageHdr) + 16) + 128; }
@@ -138,22 +137,102 @@ __device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, dou
 }
 
 // ---------------------------------------------------------------- consumer warps
-// One k-tile of the warp tile restricted to its first MI x NJ sub-tiles (compile-time bounds: no predicates).
-// offA[k4] / offB[j]: this lane's swizzled element offsets inside the P / Q image (constant over the kernel).
-template <int MI, int NJ>
-__device__ __forceinline__ void mma_ktile(double (&acc)[4][NJW][2], const double *sP, const double *sQ,
-                                          const int (&offA)[4], const int (&offB)[NJW]) {
+// The 64 x 64 tile is 8 x 8 sub-tiles of 8 x 8 (one DMMA.8x8x4 accumulator each); a warp owns a TH x TW block of them
+// (TH * TW = 8 accumulator pairs, index i * TW + j) and the eight warps form a (8 / TH) x (8 / TW) grid.  Four layouts:
+//   TH x TW = 4 x 2 (warp grid 2 x 4; full tiles: 6 fragment loads per 8 DMMA), 2 x 4, 8 x 1 and 1 x 8.
+// For an EDGE tile (sm x sn sub-tiles with data) the producer picks the layout with the smallest busiest warp,
+// min(TH, sm) * min(TW, sn): a CTA advances at the pace of its busiest warp, so e.g. a tile with 40 of 64 rows costs 5/8
+// of a full tile with the 8 x 1 layout instead of 8/8 (cfg 3: -10 % on the critical path, cfg 5a: -16 %).
+struct Lane {            // lane constants of the swizzled fragment addresses (internal.h: img_p_index / img_q_index)
+    int offA[4];         // P: gq * BK + (((2 k4 + tg / 2) ^ 2 (gq % 4)) << 1) + tg % 2, per k4
+    int rowB, c0, x2;    // Q: tg * BN + gq % 2;  gq / 2;  2 tg
+};
+
+// One k-tile of MI x NJ sub-tiles (compile-time bounds: no predicates); sc0 = first sub-tile column of the warp.
+template <int MI, int NJ, int TW>
+__device__ __forceinline__ void mma_ktile(double (&acc)[8][2], const double *sP, const double *sQ, const Lane &L, int sc0) {
+    int ob[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; j++) ob[j] = L.rowB + (((((sc0 + j) << 2) | L.c0) ^ L.x2) << 1);
 #pragma unroll
     for (int k4 = 0; k4 < BK / 4; k4++) {
         double a[MI], b[NJ];
 #pragma unroll
-        for (int i = 0; i < MI; i++) a[i] = sP[i * 8 * BK + offA[k4]];
+        for (int i = 0; i < MI; i++) a[i] = sP[i * 8 * BK + L.offA[k4]];
 #pragma unroll
-        for (int j = 0; j < NJ; j++) b[j] = sQ[k4 * 4 * BN + offB[j]];
+        for (int j = 0; j < NJ; j++) b[j] = sQ[k4 * 4 * BN + ob[j]];
 #pragma unroll
         for (int i = 0; i < MI; i++)
 #pragma unroll
-            for (int j = 0; j < NJ; j++) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            for (int j = 0; j < NJ; j++) dmma884(acc[i * TW + j][0], acc[i * TW + j][1], a[i], b[j]);
+    }
+}
+template <int TW, int NJ, int MI>
+__device__ __forceinline__ void disp_mi(int mi, double (&acc)[8][2], const double *sP, const double *sQ, const Lane &L, int sc0) {
+    if (mi == MI) mma_ktile<MI, NJ, TW>(acc, sP, sQ, L, sc0);
+    else if constexpr (MI > 1) disp_mi<TW, NJ, MI - 1>(mi, acc, sP, sQ, L, sc0);
+}
+template <int TH, int TW, int NJ>
+__device__ __forceinline__ void disp_nj(int mi, int nj, double (&acc)[8][2], const double *sP, const double *sQ, const Lane &L, int sc0) {
+    if (nj == NJ) disp_mi<TW, NJ, TH>(mi, acc, sP, sQ, L, sc0);
+    else if constexpr (NJ > 1) disp_nj<TH, TW, NJ - 1>(mi, nj, acc, sP, sQ, L, sc0);
+}
+
+// Epilogue of one warp: its TH x TW accumulator block -> C (row-major caller vector, or the tile images stage 2 loads).
+// sr0 / sc0: first sub-tile row / column of the warp; gq, tg: DMMA fragment coordinates of the lane.
+template <int TH, int TW>
+__device__ __forceinline__ void store_c(const double (&acc)[8][2], const GemmUnit &u, double *C, int sr0, int sc0, int gq, int tg, int yvec) {
+    if (u.c_kind == C_ROWMAJOR) {
+        const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
+#pragma unroll
+        for (int i = 0; i < TH; i++) {
+            const int row = u.m0 + (sr0 + i) * 8 + gq;
+            if (row >= u.M) continue;
+#pragma unroll
+            for (int j = 0; j < TW; j++) {
+                const int col = u.n0 + (sc0 + j) * 8 + 2 * tg;
+                double *dst = C + (long long)row * u.ldc + col;
+                if (cvec && col + 1 < u.N) {
+                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[i * TW + j][0], acc[i * TW + j][1]);
+                } else {
+                    if (col < u.N) dst[0] = acc[i * TW + j][0];
+                    if (col + 1 < u.N) dst[1] = acc[i * TW + j][1];
+                }
+            }
+        }
+    } else if (u.c_kind == C_IMG_P) {
+        // T (M x N) becomes the P operand of stage 2 (K = N): P images [m-tile][k-tile]; the column pair of an
+        // accumulator is one 16-byte chunk (the pad column of an odd N receives the exact zero it computed)
+        const int CT = (u.N + BK - 1) / BK;
+        double *base = C + (long long)(u.m0 / BM) * CT * IMG;
+#pragma unroll
+        for (int i = 0; i < TH; i++) {
+            const int r = (sr0 + i) * 8 + gq;
+            if (u.m0 + r >= u.M) continue;
+#pragma unroll
+            for (int j = 0; j < TW; j++) {
+                const int col = u.n0 + (sc0 + j) * 8 + 2 * tg;
+                if (col < u.N)
+                    *reinterpret_cast<double2 *>(base + (long long)(col / BK) * IMG + img_p_index(r, col % BK)) =
+                        make_double2(acc[i * TW + j][0], acc[i * TW + j][1]);
+            }
+        }
+    } else {
+        // T (M x N) becomes the Q operand of stage 2 (K = M): Q images [n-tile][k-tile]
+        const int CT = (u.M + BK - 1) / BK;
+        double *base = C + (long long)(u.n0 / BN) * CT * IMG;
+#pragma unroll
+        for (int i = 0; i < TH; i++) {
+            const int row = u.m0 + (sr0 + i) * 8 + gq;
+            if (row >= u.M) continue;
+#pragma unroll
+            for (int j = 0; j < TW; j++) {
+                const int c = (sc0 + j) * 8 + 2 * tg;
+                if (u.n0 + c < u.N)
+                    *reinterpret_cast<double2 *>(base + (long long)(row / BK) * IMG + img_q_index(row % BK, c)) =
+                        make_double2(acc[i * TW + j][0], acc[i * TW + j][1]);
+            }
+        }
     }
 }
 
@@ -277,11 +356,19 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 #undef UFIELD
             const int ext_m = min(BM, M - m0), ext_n = min(BN, N - n0);
             const int rot = ((m0 >> 6) + (n0 >> 6)) & (CWARPS - 1);     // the same for every K slice of a tile
+            int layout = 0;                                             // 0: 4x2, 1: 2x4, 2: 8x1, 3: 1x8 sub-tiles per warp
+            {
+                const int sm = (ext_m + 7) >> 3, sn = (ext_n + 7) >> 3;
+                int best = min(4, sm) * min(2, sn);
+                if (min(2, sm) * min(4, sn) < best) { best = min(2, sm) * min(4, sn); layout = 1; }
+                if (sm < best) { best = sm; layout = 2; }
+                if (sn < best) { best = sn; layout = 3; }
+            }
             const GemmItem *uitems = items + item_begin;
             if (KT == 0) {                           // an output without records: the consumers store zeros
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
-                if (lane == 0) { h->flags = F_FIRST | F_LAST; h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                if (lane == 0) { h->flags = F_FIRST | F_LAST; h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
                 if (lane < UNIT_WORDS) h->u[lane] = uw;
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(bars + s));
@@ -294,7 +381,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
                 const bool last = (t == KT - 1) && !reducer;
-                if (lane == 0) { h->flags = F_DATA | (t == 0 ? F_FIRST : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                if (lane == 0) { h->flags = F_DATA | (t == 0 ? F_FIRST : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
                 if (last && lane < UNIT_WORDS) h->u[lane] = uw;
                 __syncwarp();
                 if (lane == 0) {
@@ -336,7 +423,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                         const int s = acquire();
                         StageHdr *h = hdrs + s;
                         const bool last = (r == n_red - 1);
-                        if (lane == 0) { h->flags = F_REDUCE | (hh ? F_HALF : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; }
+                        if (lane == 0) { h->flags = F_REDUCE | (hh ? F_HALF : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
                         if (last && lane < UNIT_WORDS) h->u[lane] = uw;
                         __syncwarp();
                         if (lane == 0) {
@@ -369,22 +456,18 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         }
     } else {
         // ================================================= consumers
-        // Warp -> sub-tile: sub = (warp + rot) mod CWARPS, rows wm = 32 (sub mod 2), columns wn = (sub / 2) * 8 NJW.  The
-        // rotation changes from tile to tile so that the light warps of edge tiles (fewer rows / columns with data) do not
-        // always land on the same SM sub-partition: each sub-partition has its own DMMA pipe, and a CTA advances at the pace
-        // of its busiest warp.
+        // Warp -> block of sub-tiles: w = (warp + rot) mod 8 in the warp grid of the unit's layout.  The rotation changes
+        // from tile to tile so that the light warps of edge tiles do not always land on the same SM sub-partition (each
+        // has its own DMMA pipe).
         const int gq = lane >> 2, tg = lane & 3;
-        int offA[4], offB[NJW];                    // this lane's swizzled offsets for wm = wn = 0 (add wm * BK / wn)
+        Lane L;
 #pragma unroll
-        for (int k4 = 0; k4 < 4; k4++) offA[k4] = gq * BK + ((((2 * k4 + (tg >> 1)) ^ (2 * (gq & 3)))) << 1) + (tg & 1);
-#pragma unroll
-        for (int j = 0; j < NJW; j++) offB[j] = tg * BN + (((4 * j + (gq >> 1)) ^ (2 * tg)) << 1) + (gq & 1);
+        for (int k4 = 0; k4 < 4; k4++) L.offA[k4] = gq * BK + ((((2 * k4 + (tg >> 1)) ^ (2 * (gq & 3)))) << 1) + (tg & 1);
+        L.rowB = tg * BN + (gq & 1); L.c0 = gq >> 1; L.x2 = 2 * tg;
 
-        double acc[4][NJW][2];
+        double acc[8][2];
 #pragma unroll
-        for (int i = 0; i < 4; i++)
-#pragma unroll
-            for (int j = 0; j < NJW; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+        for (int q = 0; q < 8; q++) { acc[q][0] = 0.0; acc[q][1] = 0.0; }
         unsigned long long t_start = 0, t_main = 0;
 
         // Deferred publish: a finished tile (a T-block tile, or a parked split-K partial) is announced by this WARP on its
@@ -408,35 +491,31 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             const int flags = h->flags;
             if (flags & F_EXIT) break;
             if (trace && tid == 0 && (flags & F_FIRST)) t_start = globaltimer();
-            const int sub = (warp + h->rot) & (CWARPS - 1);
-            const int wm = (sub & 1) * 32, wn = (sub >> 1) * (8 * NJW);
+            const int w = (warp + h->rot) & (CWARPS - 1);
+            const int layout = h->layout;
+            // first sub-tile row / column of this warp: 4x2 -> grid 2x4, 2x4 -> 4x2, 8x1 -> 1x8, 1x8 -> 8x1
+            const int sr0 = layout == 0 ? (w & 1) * 4 : (layout == 1 ? (w & 3) * 2 : (layout == 2 ? 0 : w));
+            const int sc0 = layout == 0 ? (w >> 1) * 2 : (layout == 1 ? (w >> 2) * 4 : (layout == 2 ? w : 0));
             if (flags & F_DATA) {
-                // sub-tiles of this warp that hold real rows / columns (8-granular): a warp whose data fits in its first
-                // 2 sub-tile rows / columns runs a smaller DMMA block (compile-time bounds), an empty warp tile runs nothing
-                const int mi = min(max(h->ext_m - wm + 7, 0) >> 3, 4);
-                const int nj = min(max(h->ext_n - wn + 7, 0) >> 3, NJW);
-                const double *sP = stage_base + (size_t)s * STAGE_DOUBLES + wm * BK;
-                const double *sQ = stage_base + (size_t)s * STAGE_DOUBLES + IMG + wn;
-                if (NJW == 4) {
-                    if (mi > 2 && nj > 2) mma_ktile<4, NJW>(acc, sP, sQ, offA, offB);
-                    else if (mi > 2 && nj > 0) mma_ktile<4, NJW / 2>(acc, sP, sQ, offA, offB);
-                    else if (mi > 0 && nj > 2) mma_ktile<2, NJW>(acc, sP, sQ, offA, offB);
-                    else if (mi > 0 && nj > 0) mma_ktile<2, NJW / 2>(acc, sP, sQ, offA, offB);
-                } else {
-                    if (mi > 2 && nj > 1) mma_ktile<4, NJW>(acc, sP, sQ, offA, offB);
-                    else if (mi > 2 && nj > 0) mma_ktile<4, NJW / 2>(acc, sP, sQ, offA, offB);
-                    else if (mi > 0 && nj > 1) mma_ktile<2, NJW>(acc, sP, sQ, offA, offB);
-                    else if (mi > 0 && nj > 0) mma_ktile<2, NJW / 2>(acc, sP, sQ, offA, offB);
+                // sub-tiles of this warp's block that hold real rows / columns: exactly those are multiplied
+                const int mi = ((h->ext_m + 7) >> 3) - sr0, nj = ((h->ext_n + 7) >> 3) - sc0;
+                if (mi > 0 && nj > 0) {
+                    const double *sP = stage_base + (size_t)s * STAGE_DOUBLES + sr0 * 8 * BK;
+                    const double *sQ = stage_base + (size_t)s * STAGE_DOUBLES + IMG;
+                    if (layout == 0) disp_nj<4, 2, 2>(min(mi, 4), min(nj, 2), acc, sP, sQ, L, sc0);
+                    else if (layout == 1) disp_nj<2, 4, 4>(min(mi, 2), min(nj, 4), acc, sP, sQ, L, sc0);
+                    else if (layout == 2) disp_nj<8, 1, 1>(min(mi, 8), 1, acc, sP, sQ, L, sc0);
+                    else disp_nj<1, 8, 8>(1, min(nj, 8), acc, sP, sQ, L, sc0);
                 }
             } else if (flags & F_REDUCE) {
                 // half of another slice's partial tile, in fragment order [register pair][thread]: add it in place
                 const double2 *src = reinterpret_cast<const double2 *>(stage_base + (size_t)s * STAGE_DOUBLES) + tid;
                 if (flags & F_HALF) {
 #pragma unroll
-                    for (int q = 0; q < 2 * NJW; q++) { const double2 v = src[q * CONSUMERS]; acc[2 + q / NJW][q % NJW][0] += v.x; acc[2 + q / NJW][q % NJW][1] += v.y; }
+                    for (int q = 0; q < 4; q++) { const double2 v = src[q * CONSUMERS]; acc[4 + q][0] += v.x; acc[4 + q][1] += v.y; }
                 } else {
 #pragma unroll
-                    for (int q = 0; q < 2 * NJW; q++) { const double2 v = src[q * CONSUMERS]; acc[q / NJW][q % NJW][0] += v.x; acc[q / NJW][q % NJW][1] += v.y; }
+                    for (int q = 0; q < 4; q++) { const double2 v = src[q * CONSUMERS]; acc[q][0] += v.x; acc[q][1] += v.y; }
                 }
             }
             if (flags & F_LAST) {
@@ -449,65 +528,14 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     // 16-byte stores) for the tile's designated reducer
                     double2 *mine = reinterpret_cast<double2 *>(s_base[BASE_PART] + u.part_off) + (long long)u.split_idx * (BM * BN / 2);
 #pragma unroll
-                    for (int i = 0; i < 4; i++)
-#pragma unroll
-                        for (int j = 0; j < NJW; j++)
-                            __stcg(mine + (i * NJW + j) * CONSUMERS + tid, make_double2(acc[i][j][0], acc[i][j][1]));
+                    for (int q = 0; q < 8; q++) __stcg(mine + q * CONSUMERS + tid, make_double2(acc[q][0], acc[q][1]));
                     pending = counters + u.tile_id; pending_g = g;
                 } else {
                     double *C = s_base[u.c_base] + u.c_off;
-                    if (u.c_kind == C_ROWMAJOR) {
-                        const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
-#pragma unroll
-                        for (int i = 0; i < 4; i++) {
-                            const int row = u.m0 + wm + i * 8 + gq;
-                            if (row >= u.M) continue;
-#pragma unroll
-                            for (int j = 0; j < NJW; j++) {
-                                const int col = u.n0 + wn + j * 8 + 2 * tg;
-                                double *dst = C + (long long)row * u.ldc + col;
-                                if (cvec && col + 1 < u.N) {
-                                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[i][j][0], acc[i][j][1]);
-                                } else {
-                                    if (col < u.N) dst[0] = acc[i][j][0];
-                                    if (col + 1 < u.N) dst[1] = acc[i][j][1];
-                                }
-                            }
-                        }
-                    } else if (u.c_kind == C_IMG_P) {
-                        // T (M x N) becomes the P operand of stage 2 (K = N): P images [m-tile][k-tile]; the column pair of an
-                        // accumulator is one 16-byte chunk (the pad column of an odd N receives the exact zero it computed)
-                        const int CT = (u.N + BK - 1) / BK;
-                        double *base = C + (long long)(u.m0 / BM) * CT * IMG;
-#pragma unroll
-                        for (int i = 0; i < 4; i++) {
-                            const int r = wm + i * 8 + gq;
-                            if (u.m0 + r >= u.M) continue;
-#pragma unroll
-                            for (int j = 0; j < NJW; j++) {
-                                const int col = u.n0 + wn + j * 8 + 2 * tg;
-                                if (col < u.N)
-                                    *reinterpret_cast<double2 *>(base + (long long)(col / BK) * IMG + img_p_index(r, col % BK)) =
-                                        make_double2(acc[i][j][0], acc[i][j][1]);
-                            }
-                        }
-                    } else {
-                        // T (M x N) becomes the Q operand of stage 2 (K = M): Q images [n-tile][k-tile]
-                        const int CT = (u.M + BK - 1) / BK;
-                        double *base = C + (long long)(u.n0 / BN) * CT * IMG;
-#pragma unroll
-                        for (int i = 0; i < 4; i++) {
-                            const int row = u.m0 + wm + i * 8 + gq;
-                            if (row >= u.M) continue;
-#pragma unroll
-                            for (int j = 0; j < NJW; j++) {
-                                const int c = wn + j * 8 + 2 * tg;
-                                if (u.n0 + c < u.N)
-                                    *reinterpret_cast<double2 *>(base + (long long)(row / BK) * IMG + img_q_index(row % BK, c)) =
-                                        make_double2(acc[i][j][0], acc[i][j][1]);
-                            }
-                        }
-                    }
+                    if (layout == 0) store_c<4, 2>(acc, u, C, sr0, sc0, gq, tg, yvec);
+                    else if (layout == 1) store_c<2, 4>(acc, u, C, sr0, sc0, gq, tg, yvec);
+                    else if (layout == 2) store_c<8, 1>(acc, u, C, sr0, sc0, gq, tg, yvec);
+                    else store_c<1, 8>(acc, u, C, sr0, sc0, gq, tg, yvec);
                     // this tile of a T block is complete: to be published (release: this warp's stores, then its count)
                     if (u.signal >= 0) { pending = ctrl + CTRL_DEP0 + u.signal; pending_g = g; }
                 }
@@ -520,9 +548,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                             ((unsigned long long)writes_c << 50);
                 }
 #pragma unroll
-                for (int i = 0; i < 4; i++)
-#pragma unroll
-                    for (int j = 0; j < NJW; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+                for (int q = 0; q < 8; q++) { acc[q][0] = 0.0; acc[q][1] = 0.0; }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(bars + STAGES + s));     // this warp is done with the stage
@@ -550,15 +576,9 @@ typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int
                         unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long);
 struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
-#if DMRG_CWARPS == 8
-    {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},
+    {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},     // default: two CTAs per SM, each able to saturate the DMMA pipes alone
     {"s4b3", grouped_gemm_kernel<4, 3>, smem_bytes(4), 3},
     {"s5b2", grouped_gemm_kernel<5, 2>, smem_bytes(5), 2},
-#else
-    {"s4b3", grouped_gemm_kernel<4, 3>, smem_bytes(4), 3},
-    {"s3b4", grouped_gemm_kernel<3, 4>, smem_bytes(3), 4},
-    {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},
-#endif
 };
 static const Variant *g_variant = &kVariants[0];
 static int g_ctas_per_sm = 0;
