@@ -96,6 +96,9 @@ typedef struct {
     int32_t  tile;      /* projection tile selector: 0 = auto                            */
     int32_t  check_every; /* dmrg_lowest_eigenpair: host reads the device convergence flag
                              every this many iterations (0 = default 8)                   */
+    int32_t  max_rhs;     /* largest number of vectors one projection launch takes
+                             (dmrg_apply_H_multi, block Davidson): 1..4, 0 = 1.  The per-apply
+                             workspaces are allocated max_rhs times at plan creation.       */
 } dmrg_options;
 
 typedef struct {
@@ -214,6 +217,38 @@ int dmrg_ritz_vector(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
 int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag,
                           double *x_out, double *lambda, double *resnorm, int32_t *iters,
                           void *cuda_stream);
+
+/* ---- several vectors at once: block Davidson (Davidson-Liu) ------------ */
+
+/* Y(:,r) = H_SB X(:,r), r < nrhs <= options.max_rhs, in ONE grouped launch (ticket = unit * nrhs + r).  x, y DEVICE,
+ * column-contiguous with column strides ldx, ldy >= n; must not overlap.  Asynchronous, no allocation. */
+int dmrg_apply_H_multi(dmrg_handle_t h, int32_t nrhs, const double *x, int64_t ldx, double *y, int64_t ldy,
+                       void *cuda_stream);
+
+/* Block iteration for the nb lowest eigenpairs (1 <= nb <= options.max_rhs, 2 nb <= k_max), the textbook method in
+ * the line order of Alg. 3 with nb columns where Alg. 3 has one (readings A29-A32):
+ *   init:  V(:,0..nb-1) = orthonormalised X0 (thin QR, positive diagonal); k = na = nb.   X0 DEVICE n x nb, stride ldx0.
+ *   step:  W(:,new) = H_SB V(:,new) for the *na newest columns (one launch); G(:,new) = V^T W(:,new);
+ *          (theta_i, y_i) the nb lowest eigenpairs of G; x_i = V y_i; r_i = W y_i - theta_i x_i;
+ *          converged when every ||r_i|| <= tol; otherwise one correction t_i = r_i / g(theta_i - D) per pair that is NOT
+ *          converged, restart (collapse to the nb Ritz vectors) when they would not fit, Gram-Schmidt against V
+ *          (options.reorth passes) and among themselves, append.  *k and *na (number of appended columns, still to be
+ *          projected) are updated; theta, resnorm: HOST arrays of nb.  Synchronises the stream.
+ *   ritz:  X_out(:,i) = V y_i / ||V y_i|| with the y_i of the last step (k = basis size of that step).
+ * V, W as in dmrg_davidson_init.  DMRG_E_NUMERIC: dependent or non-finite vectors. */
+int dmrg_block_init(dmrg_handle_t h, int32_t nb, const double *X0, int64_t ldx0, double *V, double *W, int64_t ldv,
+                    void *cuda_stream);
+int dmrg_block_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, int32_t *na, int32_t nb,
+                    double *theta, double *resnorm, int32_t *converged, void *cuda_stream);
+int dmrg_block_ritz(dmrg_handle_t h, const double *V, const double *W, int64_t ldv, int32_t k, int32_t nb,
+                    double *X_out, int64_t ldxo, void *cuda_stream);
+/* Small-matrix state of the last block step: G (k_max x k_max, row-major) and Y (k_max x nb, row-major) to HOST. */
+int dmrg_block_get_small(dmrg_handle_t h, int32_t nb, double *G_host, double *Y_host, void *cuda_stream);
+/* Driver: the nb lowest eigenpairs from the start block X0 (DEVICE n x nb), on plan-owned V, W.  X_out DEVICE n x nb
+ * (stride ldxo); theta, resnorm HOST nb; iters = block iterations, applies = projections of single vectors. */
+int dmrg_block_lowest_eigenpairs(dmrg_handle_t h, int32_t nb, const double *X0, int64_t ldx0, double *X_out,
+                                 int64_t ldxo, double *theta, double *resnorm, int32_t *iters, int32_t *applies,
+                                 void *cuda_stream);
 
 /* ---- the Davidson BLAS-2 kernels on their own (Alg. 3 lines 3, 5-6, 12-13; Alg. 4) --- */
 

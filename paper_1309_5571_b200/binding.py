@@ -24,6 +24,8 @@ EXPORTS = [
     "dmrg_last_error", "dmrg_apply_H", "dmrg_davidson_init", "dmrg_davidson_step", "dmrg_davidson_step_host", "dmrg_davidson_poll", "dmrg_get_small",
     "dmrg_set_small", "dmrg_ritz_vector", "dmrg_lowest_eigenpair", "dmrg_gemv_trans", "dmrg_gemv_sub",
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
+    "dmrg_apply_H_multi", "dmrg_block_init", "dmrg_block_step", "dmrg_block_ritz", "dmrg_block_get_small",
+    "dmrg_block_lowest_eigenpairs",
 ]
 
 
@@ -54,7 +56,7 @@ class _Problem(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("tol", C.c_double), ("max_iter", C.c_int32), ("reorth", C.c_int32),
-                ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32)]
+                ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32), ("max_rhs", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -106,6 +108,12 @@ def load_library():
         "dmrg_get_timing": [vp, pdbl],
         "dmrg_get_unit_trace": [vp, C.POINTER(C.c_uint64), i32, pi32],
         "dmrg_version": [],
+        "dmrg_apply_H_multi": [vp, i32, vp, i64, vp, i64, vp],
+        "dmrg_block_init": [vp, i32, vp, i64, vp, vp, i64, vp],
+        "dmrg_block_step": [vp, vp, vp, i64, pi32, pi32, i32, pdbl, pdbl, pi32, vp],
+        "dmrg_block_ritz": [vp, vp, vp, i64, i32, i32, vp, i64, vp],
+        "dmrg_block_get_small": [vp, i32, pdbl, pdbl, vp],
+        "dmrg_block_lowest_eigenpairs": [vp, i32, vp, i64, vp, i64, pdbl, pdbl, pi32, pi32, vp],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -146,7 +154,7 @@ class Plan:
     """Owns a dmrg_handle_t plus the device copies of the operator blocks."""
 
     def __init__(self, problem, k_max: int = 20, tol: float = 1e-10, max_iter: int = 2000, reorth: int = 1,
-                 seed: int = 1, check_every: int = 8, device: Optional[str] = None):
+                 seed: int = 1, check_every: int = 8, max_rhs: int = 1, device: Optional[str] = None):
         torch = _torch()
         self._lib = load_library()
         self._keep = []
@@ -163,7 +171,7 @@ class Plan:
         tgt = np.ascontiguousarray(np.asarray(problem.target, dtype=np.int32).ravel())
         self._keep.append(tgt)
         pr.target = tgt.ctypes.data_as(C.POINTER(C.c_int32))
-        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every))
+        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(max_rhs))
         h = C.c_void_p()
         rc = self._lib.dmrg_plan_create(C.byref(pr), C.byref(opt), C.byref(h))
         if rc != DMRG_OK:
@@ -238,7 +246,84 @@ class Plan:
         self._check(self._lib.dmrg_apply_H(self._h, _ptr(x), _ptr(y), _stream_ptr(stream)))
         return y
 
+    # ---- several vectors at once (block Davidson).  Blocks of vectors are (nb, ld) row-major tensors =
+    #      column-contiguous n x nb, like V and W.
+    def _check_block(self, X, nb: int, name: str) -> int:
+        if X.dim() != 2 or X.shape[0] < nb or X.stride(1) != 1 or X.stride(0) < self.n or not X.is_cuda or X.dtype != _torch().float64:
+            raise ValueError(f"{name}: need a float64 CUDA tensor of shape (>= {nb}, ld >= n) with contiguous rows")
+        return int(X.stride(0))
+
+    def apply_H_multi(self, X, Y=None, stream=None):
+        torch = _torch()
+        nb = X.shape[0]
+        ldx = self._check_block(X, nb, "X")
+        if Y is None:
+            Y = torch.empty((nb, (self.n + 15) // 16 * 16), dtype=torch.float64, device=self.device)
+        ldy = self._check_block(Y, nb, "Y")
+        self._check(self._lib.dmrg_apply_H_multi(self._h, int(nb), _ptr(X), ldx, _ptr(Y), ldy, _stream_ptr(stream)))
+        return Y
+
+    def block_init(self, V, W, X0, stream=None):
+        nb = X0.shape[0]
+        ldx = self._check_block(X0, nb, "X0")
+        self._check_basis(V, W)
+        self._check(self._lib.dmrg_block_init(self._h, int(nb), _ptr(X0), ldx, _ptr(V), _ptr(W), int(V.stride(0)), _stream_ptr(stream)))
+        return nb, nb
+
+    def block_step(self, V, W, k: int, na: int, nb: int, stream=None):
+        """-> (k, na, theta[nb], resnorm[nb], converged)"""
+        self._check_basis(V, W)
+        kk, nn, conv = C.c_int32(int(k)), C.c_int32(int(na)), C.c_int32()
+        th = (C.c_double * nb)(); rho = (C.c_double * nb)()
+        self._check(self._lib.dmrg_block_step(self._h, _ptr(V), _ptr(W), int(V.stride(0)), C.byref(kk), C.byref(nn), int(nb),
+                                              th, rho, C.byref(conv), _stream_ptr(stream)))
+        return int(kk.value), int(nn.value), np.array(th[:]), np.array(rho[:]), bool(conv.value)
+
+    def block_ritz(self, V, W, k: int, nb: int, stream=None):
+        torch = _torch()
+        X = torch.empty((nb, (self.n + 15) // 16 * 16), dtype=torch.float64, device=self.device)
+        self._check(self._lib.dmrg_block_ritz(self._h, _ptr(V), _ptr(W), int(V.stride(0)), int(k), int(nb), _ptr(X), int(X.stride(0)),
+                                              _stream_ptr(stream)))
+        return X[:, :self.n]
+
+    def block_get_small(self, nb: int, stream=None):
+        G = np.zeros((self.k_max, self.k_max)); Y = np.zeros((self.k_max, nb))
+        self._check(self._lib.dmrg_block_get_small(self._h, int(nb), G.ctypes.data_as(C.POINTER(C.c_double)),
+                                                   Y.ctypes.data_as(C.POINTER(C.c_double)), _stream_ptr(stream)))
+        return G, Y
+
+    def block_lowest_eigenpairs(self, X0, stream=None):
+        """-> (rc, theta[nb], X (nb, n), resnorm[nb], block iterations, applies)"""
+        torch = _torch()
+        nb = X0.shape[0]
+        ldx = self._check_block(X0, nb, "X0")
+        X = torch.empty((nb, (self.n + 15) // 16 * 16), dtype=torch.float64, device=self.device)
+        th = (C.c_double * nb)(); rho = (C.c_double * nb)(); it = C.c_int32(); ap = C.c_int32()
+        rc = self._lib.dmrg_block_lowest_eigenpairs(self._h, int(nb), _ptr(X0), ldx, _ptr(X), int(X.stride(0)), th, rho,
+                                                    C.byref(it), C.byref(ap), _stream_ptr(stream))
+        if rc < 0:
+            self._check(rc)
+        return rc, np.array(th[:]), X[:, :self.n], np.array(rho[:]), int(it.value), int(ap.value)
+
+    def _check_basis(self, V, W):
+        """a wrong-shaped basis must not reach the kernels (they would write out of bounds)."""
+        t = _torch()
+        for nm, B in (("V", V), ("W", W)):
+            if not (isinstance(B, t.Tensor) and B.is_cuda and B.dtype == t.float64 and B.dim() == 2 and B.shape[0] >= self.k_max
+                    and B.stride(1) == 1 and B.stride(0) >= self.n):
+                raise ValueError(f"{nm}: need a float64 CUDA tensor of shape (>= k_max, ld >= n) with contiguous rows "
+                                 f"(column-contiguous n x k_max), got {tuple(B.shape) if hasattr(B, 'shape') else type(B)}")
+        if V.stride(0) != W.stride(0):
+            raise ValueError("V and W must have the same column stride")
+
+    def _check_cols(self, V, k: int):
+        t = _torch()
+        if not (isinstance(V, t.Tensor) and V.is_cuda and V.dtype == t.float64 and V.dim() == 2 and V.shape[0] >= k
+                and V.stride(1) == 1 and V.stride(0) >= self.n):
+            raise ValueError(f"V: need a float64 CUDA tensor of shape (>= {k}, ld >= n) with contiguous rows")
+
     def davidson_init(self, V, W, x0=None, start_at_argmin_diag: bool = False, stream=None):
+        self._check_basis(V, W)
         if x0 is not None:
             _check_vec(x0, self.n, "x0")
         ldv = V.stride(0) if V.dim() == 2 else self.n
@@ -247,6 +332,7 @@ class Plan:
 
     def davidson_enqueue(self, V, W, k: int, stream=None) -> int:
         """dmrg_davidson_step with NULL outputs: enqueue only, returns the next basis size; see davidson_poll."""
+        self._check_basis(V, W)
         kk = C.c_int32(int(k))
         ldv = V.stride(0) if V.dim() == 2 else self.n
         self._check(self._lib.dmrg_davidson_step(self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), None, None, None,
@@ -262,6 +348,7 @@ class Plan:
 
     def davidson_step_host(self, V, W, k: int, v_in_host=None, w_out_host=None, stream=None) -> Tuple[int, float, float, bool]:
         """dmrg_davidson_step_host: v_in_host / w_out_host are CPU float64 tensors of n elements (pinned for overlap)."""
+        self._check_basis(V, W)
         for nm, t in (("v_in_host", v_in_host), ("w_out_host", w_out_host)):
             if t is not None and (t.is_cuda or t.dtype != _torch().float64 or t.numel() != self.n or not t.is_contiguous()):
                 raise ValueError(f"{nm} must be a contiguous CPU float64 tensor of {self.n} elements")
@@ -273,6 +360,7 @@ class Plan:
         return int(kk.value), float(lam.value), float(rho.value), bool(conv.value)
 
     def davidson_step(self, V, W, k: int, stream=None) -> Tuple[int, float, float, bool]:
+        self._check_basis(V, W)
         kk, lam, rho, conv = C.c_int32(int(k)), C.c_double(), C.c_double(), C.c_int32()
         ldv = V.stride(0) if V.dim() == 2 else self.n
         self._check(self._lib.dmrg_davidson_step(self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), C.byref(lam),
@@ -291,6 +379,7 @@ class Plan:
         self._check(self._lib.dmrg_set_small(self._h, B.ctypes.data_as(C.POINTER(C.c_double)), _stream_ptr()))
 
     def ritz_vector(self, V, k: int, stream=None):
+        self._check_cols(V, k)
         torch = _torch()
         x = torch.empty(self.n, dtype=torch.float64, device=self.device)
         ldv = V.stride(0) if V.dim() == 2 else self.n
@@ -310,6 +399,7 @@ class Plan:
         return rc, float(lam.value), x_out, float(rho.value), int(it.value)
 
     def gemv_trans(self, V, k: int, w, out=None, stream=None):
+        self._check_cols(V, k)
         torch = _torch()
         if out is None:
             out = torch.empty(k, dtype=torch.float64, device=self.device)
@@ -318,6 +408,7 @@ class Plan:
         return out
 
     def gemv_sub(self, V, k: int, s, t, nrm2=None, stream=None):
+        self._check_cols(V, k)
         torch = _torch()
         if nrm2 is None:
             nrm2 = torch.empty(1, dtype=torch.float64, device=self.device)

@@ -211,6 +211,18 @@ int dmrg_ritz_vector(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, d
     return dav_ritz(p, V, ldv, k, x_out, S(stream));
 }
 
+static int ensure_own_basis(Plan *p) {
+    if (p->Vown) return DMRG_OK;
+    p->ldv_own = (p->n + 15) / 16 * 16;
+    size_t bytes = sizeof(double) * (size_t)p->ldv_own * p->opt.k_max;
+    if (cudaMalloc((void **)&p->Vown, bytes) != cudaSuccess || cudaMalloc((void **)&p->Wown, bytes) != cudaSuccess) {
+        cudaFree(p->Vown); p->Vown = nullptr; p->Wown = nullptr; cudaGetLastError();
+        return fail(p, DMRG_E_ALLOC, "cannot allocate the plan-owned Davidson basis");
+    }
+    p->device_bytes += 2 * (long long)bytes;
+    return DMRG_OK;
+}
+
 int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag, double *x_out,
                           double *lambda, double *resnorm, int32_t *iters, void *stream) {
     if (!h) return DMRG_E_INVALID_ARG;
@@ -218,15 +230,7 @@ int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_ar
     if (!x_out) return fail(p, DMRG_E_INVALID_ARG, "lowest_eigenpair: x_out is NULL");
     cudaStream_t st = S(stream);
     const int k_max = p->opt.k_max;
-    if (!p->Vown) {
-        p->ldv_own = (p->n + 15) / 16 * 16;
-        size_t bytes = sizeof(double) * (size_t)p->ldv_own * k_max;
-        if (cudaMalloc((void **)&p->Vown, bytes) != cudaSuccess || cudaMalloc((void **)&p->Wown, bytes) != cudaSuccess) {
-            cudaFree(p->Vown); p->Vown = nullptr; p->Wown = nullptr; cudaGetLastError();
-            return fail(p, DMRG_E_ALLOC, "lowest_eigenpair: cannot allocate the Davidson basis");
-        }
-        p->device_bytes += 2 * (long long)bytes;
-    }
+    { int rcb = ensure_own_basis(p); if (rcb != DMRG_OK) return rcb; }
     const bool was_timing = p->timing.enabled;
     p->timing.enabled = false;
     int rc = dav_init(p, x0, start_at_argmin_diag, p->Vown, p->Wown, p->ldv_own, st);
@@ -259,6 +263,76 @@ int dmrg_lowest_eigenpair(dmrg_handle_t h, const double *x0, int32_t start_at_ar
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
     return done == 1 ? DMRG_OK : DMRG_NOT_CONVERGED;
+}
+
+int dmrg_apply_H_multi(dmrg_handle_t h, int32_t nrhs, const double *x, int64_t ldx, double *y, int64_t ldy, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!x || !y || ldx < p->n || ldy < p->n) return fail(p, DMRG_E_INVALID_ARG, "apply_H_multi: NULL vectors or a column stride below n");
+    const double *xe = x + (nrhs - 1) * ldx + p->n; const double *ye = y + (nrhs - 1) * ldy + p->n;
+    if (!(xe <= y || ye <= x)) return fail(p, DMRG_E_INVALID_ARG, "apply_H_multi: x and y overlap");
+    return apply_H(p, x, y, nullptr, S(stream), nullptr, nrhs, ldx, ldy);
+}
+
+int dmrg_block_init(dmrg_handle_t h, int32_t nb, const double *X0, int64_t ldx0, double *V, double *W, int64_t ldv, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    return bdav_init(P(h), nb, X0, ldx0, V, W, ldv, S(stream));
+}
+
+int dmrg_block_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, int32_t *na, int32_t nb, double *theta,
+                    double *resnorm, int32_t *converged, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || !k || !na) return fail(p, DMRG_E_INVALID_ARG, "block_step: NULL argument");
+    int kk = *k, nn = *na;
+    int rc = bdav_step(p, V, W, ldv, &kk, &nn, nb, theta, resnorm, converged, S(stream));
+    if (rc == DMRG_OK) { *k = kk; *na = nn; }
+    return rc;
+}
+
+int dmrg_block_ritz(dmrg_handle_t h, const double *V, const double *W, int64_t ldv, int32_t k, int32_t nb, double *X_out,
+                    int64_t ldxo, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    if (!V || !W || !X_out) return fail(P(h), DMRG_E_INVALID_ARG, "block_ritz: NULL argument");
+    return bdav_ritz(P(h), V, W, ldv, k, nb, X_out, ldxo, S(stream));
+}
+
+int dmrg_block_get_small(dmrg_handle_t h, int32_t nb, double *G_host, double *Y_host, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!p->bstate || nb < 1 || nb > BMAX) return fail(p, DMRG_E_INVALID_ARG, "block_get_small: no block state (options.max_rhs) or bad nb");
+    cudaError_t e = cudaMemcpyAsync(p->bstate_host, p->bstate, sizeof(BlockState), cudaMemcpyDeviceToHost, S(stream));
+    if (e == cudaSuccess) e = cudaStreamSynchronize(S(stream));
+    if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    const int km = p->opt.k_max;
+    if (G_host) for (int i = 0; i < km; i++) for (int j = 0; j < km; j++) G_host[i * km + j] = p->bstate_host->G[i * KMAX + j];
+    if (Y_host) for (int i = 0; i < km; i++) for (int r = 0; r < nb; r++) Y_host[i * nb + r] = p->bstate_host->Y[i * BMAX + r];
+    return DMRG_OK;
+}
+
+int dmrg_block_lowest_eigenpairs(dmrg_handle_t h, int32_t nb, const double *X0, int64_t ldx0, double *X_out, int64_t ldxo,
+                                 double *theta, double *resnorm, int32_t *iters, int32_t *applies, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!X_out) return fail(p, DMRG_E_INVALID_ARG, "block_lowest_eigenpairs: X_out is NULL");
+    int rc = ensure_own_basis(p);
+    if (rc != DMRG_OK) return rc;
+    cudaStream_t st = S(stream);
+    rc = bdav_init(p, nb, X0, ldx0, p->Vown, p->Wown, p->ldv_own, st);
+    int k = nb, na = nb, it = 0, ap = 0, conv = 0, k_used = nb;
+    while (rc == DMRG_OK && ap < p->opt.max_iter) {
+        it++; ap += na; k_used = k;
+        rc = bdav_step(p, p->Vown, p->Wown, p->ldv_own, &k, &na, nb, theta, resnorm, &conv, st);
+        if (conv) break;
+    }
+    if (iters) *iters = it;
+    if (applies) *applies = ap;
+    if (rc != DMRG_OK) return rc;
+    rc = bdav_ritz(p, p->Vown, p->Wown, p->ldv_own, k_used, nb, X_out, ldxo, st);
+    if (rc != DMRG_OK) return rc;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
+    return conv ? DMRG_OK : DMRG_NOT_CONVERGED;
 }
 
 int dmrg_gemv_trans(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, const double *w, double *out, void *stream) {

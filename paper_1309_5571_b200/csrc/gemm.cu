@@ -44,7 +44,7 @@ enum : int { F_DATA = 1, F_LAST = 2, F_EXIT = 4, F_FIRST = 8, F_REDUCE = 16, F_H
 constexpr int PUBLISH_DELAY = 2;           // stages a consumer warp works on before it fences and signals a finished tile
 struct StageHdr {
     int flags, ticket, ext_m, ext_n;       // ext: rows / columns of the 64x64 tile that hold data
-    int rot, layout, pad[2];               // sub-tile rotation and warp layout of the unit (see the consumers)
+    int rot, layout, rhs, pad;             // sub-tile rotation and warp layout of the unit (see the consumers); right-hand side
     int u[UNIT_WORDS];                     // the unit descriptor (valid in the unit's last stage: epilogue)
 };
 constexpr int smem_bytes(int stages) { return stages * (STAGE_DOUBLES * 8 + (int)sizeof(StageHdr) + 16) + 128; }
@@ -114,13 +114,13 @@ struct Producer {
     int K, k0;                 // item K; k0 of the next tile to produce
 };
 
-__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, int m0, int n0, int k0,
-                                           int lane, const int *ctrl, int *err) {
+__device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, const long long *stride,
+                                           int rhs, int n_deps, int m0, int n0, int k0, int lane, const int *ctrl, int *err) {
     const int dep = it->dep;
     if (dep >= 0) {            // operand is a T block of this launch: wait until all its tiles are written
         if (lane == 0) {
             const int need = it->dep_need;
-            const int *c = ctrl + CTRL_DEP0 + dep;
+            const int *c = ctrl + CTRL_DEP0 + rhs * n_deps + dep;
             long long spins = 0;
             while (ld_acquire(c) < need) {
                 __nanosleep(32);
@@ -132,8 +132,8 @@ __device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, dou
     }
     pr.K = it->K; pr.k0 = k0;
     const int KT = (pr.K + BK - 1) / BK;
-    pr.pP = bases[it->p_base] + it->p_off + ((long long)(m0 / BM) * KT + k0 / BK) * IMG;
-    pr.pQ = bases[it->q_base] + it->q_off + ((long long)(n0 / BN) * KT + k0 / BK) * IMG;
+    pr.pP = bases[it->p_base] + rhs * stride[it->p_base] + it->p_off + ((long long)(m0 / BM) * KT + k0 / BK) * IMG;
+    pr.pQ = bases[it->q_base] + rhs * stride[it->q_base] + it->q_off + ((long long)(n0 / BN) * KT + k0 / BK) * IMG;
 }
 
 // ---------------------------------------------------------------- consumer warps
@@ -277,13 +277,14 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
                     const int *__restrict__ done_flag, int yvec, unsigned long long *__restrict__ trace,
                     Prefetch pf, int *__restrict__ err, const XSeg *__restrict__ xsegs, int n_xsegs,
-                    const double *__restrict__ x, long long n) {
+                    const double *__restrict__ x, long long n, RhsInfo rh) {
     if (done_flag && *done_flag) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *stage_base = reinterpret_cast<double *>(smem_raw);
     StageHdr *hdrs = reinterpret_cast<StageHdr *>(smem_raw + (size_t)STAGES * STAGE_DOUBLES * 8);
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(hdrs + STAGES);     // full[STAGES], empty[STAGES]
     __shared__ double *s_base[BASE_COUNT];      // dynamically indexed: shared memory, not a local-memory copy of the parameter
+    __shared__ long long s_stride[BASE_COUNT];  // distance between the copies of a buffer for consecutive right-hand sides
     __shared__ int s_is_last;                   // end of the launch only
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -295,8 +296,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
-    if (tid < BASE_COUNT) s_base[tid] = bases.p[tid];
-    unsigned long long *ctr = trace ? trace + 4ull * n_units + 4ull * blockIdx.x : nullptr;   // per-CTA phase stamps (diagnostics)
+    if (tid < BASE_COUNT) { s_base[tid] = bases.p[tid]; s_stride[tid] = rh.stride[tid]; }
+    const int nrhs = rh.nrhs;
+    unsigned long long *ctr = trace ? trace + 4ull * n_units * nrhs + 4ull * blockIdx.x : nullptr;   // per-CTA phase stamps (diagnostics)
     if (ctr && tid == 0) ctr[0] = globaltimer();
     // Phase 0: the caller's vector -> tile images (both operand roles), shared out over all CTAs; a CTA publishes its share
     // (CTRL_XREADY) and the producers wait for all shares before their first copy.  Every CTA of the grid is resident
@@ -311,7 +313,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             __syncthreads();
             segs = reinterpret_cast<const XSeg *>(smem_raw);
         }
-        ximg_share(segs, n_xsegs, x, lo, min(n, lo + share), bases.p[BASE_XP], bases.p[BASE_XQ], tid);
+        for (int r = 0; r < nrhs; r++)
+            ximg_share(segs, n_xsegs, x + r * rh.x_ld, lo, min(n, lo + share), bases.p[BASE_XP] + r * rh.stride[BASE_XP],
+                       bases.p[BASE_XQ] + r * rh.stride[BASE_XQ], tid);
     }
     fence_proxy_async();
     __threadfence();
@@ -341,8 +345,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             int ticket = 0;
             if (lane == 0) ticket = atomicAdd(&ctrl[CTRL_TICKET], 1);
             ticket = __shfl_sync(0xffffffffu, ticket, 0);
-            if (ticket >= n_units) break;
-            const int uw = lane < UNIT_WORDS ? reinterpret_cast<const int *>(units + ticket)[lane] : 0;
+            if (ticket >= n_units * nrhs) break;
+            const int rhs = ticket % nrhs;               // ticket = unit * nrhs + rhs: a unit waits on smaller tickets only
+            const int uw = lane < UNIT_WORDS ? reinterpret_cast<const int *>(units + ticket / nrhs)[lane] : 0;
 #define UFIELD(f) __shfl_sync(0xffffffffu, uw, (int)(offsetof(GemmUnit, f) / 4))
             const int M = UFIELD(M), N = UFIELD(N), m0 = UFIELD(m0), n0 = UFIELD(n0);
             (void)0;
@@ -368,7 +373,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             if (KT == 0) {                           // an output without records: the consumers store zeros
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
-                if (lane == 0) { h->flags = F_FIRST | F_LAST; h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
+                if (lane == 0) { h->flags = F_FIRST | F_LAST; h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; h->rhs = rhs; }
                 if (lane < UNIT_WORDS) h->u[lane] = uw;
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(bars + s));
@@ -376,12 +381,12 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 continue;
             }
             Producer pr{};
-            begin_item(pr, uitems + p_item, s_base, m0, n0, k00, lane, ctrl, err);
+            begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, k00, lane, ctrl, err);
             for (int t = 0; t < KT; t++) {
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
                 const bool last = (t == KT - 1) && !reducer;
-                if (lane == 0) { h->flags = F_DATA | (t == 0 ? F_FIRST : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
+                if (lane == 0) { h->flags = F_DATA | (t == 0 ? F_FIRST : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; h->rhs = rhs; }
                 if (last && lane < UNIT_WORDS) h->u[lane] = uw;
                 __syncwarp();
                 if (lane == 0) {
@@ -394,7 +399,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 g++;
                 if (pr.k0 >= pr.K && t + 1 < KT) {
                     p_item++;
-                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, m0, n0, 0, lane, ctrl, err);
+                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, 0, lane, ctrl, err);
                 }
             }
             if (reducer) {
@@ -403,7 +408,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 // through the ring -- 32 KB per slice = two stages -- and let the consumers add them to their registers IN
                 // SLICE ORDER (fixed at plan time: bitwise independent of timing, A22/A23).  The wait is on smaller tickets only.
                 if (lane == 0) {
-                    int *c = counters + tile_id;
+                    int *c = counters + rhs * rh.n_counters + tile_id;
                     const int need = CWARPS * (n_split - 1);
                     long long spins = 0;
                     while (ld_acquire(c) < need) {
@@ -414,7 +419,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 }
                 __syncwarp();
                 fence_proxy_async();
-                const double *part = s_base[BASE_PART] + (((long long)part_hi << 32) | (unsigned)part_lo);
+                const double *part = s_base[BASE_PART] + rhs * s_stride[BASE_PART] + (((long long)part_hi << 32) | (unsigned)part_lo);
                 const int n_red = 2 * (n_split - 1);
                 int r = 0;
                 for (int sl = 0; sl < n_split; sl++) {
@@ -423,7 +428,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                         const int s = acquire();
                         StageHdr *h = hdrs + s;
                         const bool last = (r == n_red - 1);
-                        if (lane == 0) { h->flags = F_REDUCE | (hh ? F_HALF : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; }
+                        if (lane == 0) { h->flags = F_REDUCE | (hh ? F_HALF : 0) | (last ? F_LAST : 0); h->ticket = ticket; h->ext_m = ext_m; h->ext_n = ext_n; h->rot = rot; h->layout = layout; h->rhs = rhs; }
                         if (last && lane < UNIT_WORDS) h->u[lane] = uw;
                         __syncwarp();
                         if (lane == 0) {
@@ -526,18 +531,19 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 if (!writes_c) {
                     // split K, not the reducer: park the partial tile (fragment order: [slice][register pair][thread], coalesced
                     // 16-byte stores) for the tile's designated reducer
-                    double2 *mine = reinterpret_cast<double2 *>(s_base[BASE_PART] + u.part_off) + (long long)u.split_idx * (BM * BN / 2);
+                    double2 *mine = reinterpret_cast<double2 *>(s_base[BASE_PART] + h->rhs * s_stride[BASE_PART] + u.part_off) +
+                                    (long long)u.split_idx * (BM * BN / 2);
 #pragma unroll
                     for (int q = 0; q < 8; q++) __stcg(mine + q * CONSUMERS + tid, make_double2(acc[q][0], acc[q][1]));
-                    pending = counters + u.tile_id; pending_g = g;
+                    pending = counters + h->rhs * rh.n_counters + u.tile_id; pending_g = g;
                 } else {
-                    double *C = s_base[u.c_base] + u.c_off;
+                    double *C = s_base[u.c_base] + h->rhs * s_stride[u.c_base] + u.c_off;
                     if (layout == 0) store_c<4, 2>(acc, u, C, sr0, sc0, gq, tg, yvec);
                     else if (layout == 1) store_c<2, 4>(acc, u, C, sr0, sc0, gq, tg, yvec);
                     else if (layout == 2) store_c<8, 1>(acc, u, C, sr0, sc0, gq, tg, yvec);
                     else store_c<1, 8>(acc, u, C, sr0, sc0, gq, tg, yvec);
                     // this tile of a T block is complete: to be published (release: this warp's stores, then its count)
-                    if (u.signal >= 0) { pending = ctrl + CTRL_DEP0 + u.signal; pending_g = g; }
+                    if (u.signal >= 0) { pending = ctrl + CTRL_DEP0 + h->rhs * n_deps + u.signal; pending_g = g; }
                 }
                 if (trace && tid == 0) {
                     unsigned long long *tr = trace + 4ull * h->ticket;
@@ -565,7 +571,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     }
     __syncthreads();
     if (s_is_last) {
-        for (int e = tid; e < CTRL_DEP0 + n_deps; e += THREADS) ctrl[e] = 0;
+        for (int e = tid; e < CTRL_DEP0 + n_deps * nrhs; e += THREADS) ctrl[e] = 0;
     }
 }
 
@@ -573,7 +579,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
 typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int,
-                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long);
+                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo);
 struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
     {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},     // default: two CTAs per SM, each able to saturate the DMMA pipes alone
@@ -599,7 +605,9 @@ cudaError_t gemm_kernel_setup() {
     return cudaSuccess;
 }
 
-int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in) {
+int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in,
+            int nrhs, long long ldx, long long ldy) {
+    if (nrhs < 1 || nrhs > p->max_rhs) return fail(p, DMRG_E_INVALID_ARG, "apply_H: more right-hand sides than options.max_rhs");
     BasePtrs b;
     b.p[BASE_XP] = p->ximg_p;
     b.p[BASE_XQ] = p->ximg_q;
@@ -612,13 +620,17 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
     const int n_units = p->n_units1 + p->n_units2;
     p->launches += n_units > 0 ? 1 : 0;
     if (n_units > 0) {
-        const int yvec = ((reinterpret_cast<uintptr_t>(y) & 15) == 0) ? 1 : 0;
+        const int yvec = ((reinterpret_cast<uintptr_t>(y) & 15) == 0 && (nrhs == 1 || ldy % 2 == 0)) ? 1 : 0;
+        RhsInfo rh{};
+        rh.nrhs = nrhs; rh.n_deps = p->n_deps; rh.n_counters = p->n_counters; rh.x_ld = ldx;
+        rh.stride[BASE_XP] = p->xp_elems; rh.stride[BASE_XQ] = p->xq_elems; rh.stride[BASE_T] = p->tws_elems;
+        rh.stride[BASE_PART] = p->part_elems; rh.stride[BASE_Y] = ldy; rh.stride[BASE_POOL] = 0;
         Prefetch pf;
         if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) pf = *pf_in;
-        const int grid = std::min(n_units, g_ctas_per_sm * p->sm_count);     // persistent: one wave, units by ticket
+        const int grid = (int)std::min<long long>((long long)n_units * nrhs, (long long)g_ctas_per_sm * p->sm_count);   // persistent: one wave
         g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
                                                               p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
-                                                              p->xsegs, p->n_xsegs, x, p->n);
+                                                              p->xsegs, p->n_xsegs, x, p->n, rh);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

@@ -58,6 +58,10 @@ struct GemmUnit {
 enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_XREADY = 2, CTRL_DEP0 = 3 };   // XREADY: CTAs whose share of the X images is written
 
 struct BasePtrs { double *p[BASE_COUNT]; };
+// Several right-hand sides in ONE grouped launch (block Davidson): ticket = unit * nrhs + rhs; every
+// per-apply buffer and counter set exists once per right-hand side, `stride` elements (or counters) apart.
+constexpr int BMAX = 4;         // largest block size
+struct RhsInfo { int nrhs, n_deps, n_counters, pad; long long stride[BASE_COUNT]; long long x_ld; };
 
 // tile shape of the grouped kernel (gemm.cu is compiled for exactly these)
 constexpr int BM = 64, BN = 64, BK = 16;
@@ -109,6 +113,16 @@ struct DavState {
     int pad[1];
 };
 
+// ---- block Davidson device state (oracle/block_davidson.py)
+struct BlockState {
+    double G[KMAX * KMAX];       // V^T W, row-major, symmetric (the paper's B)
+    double Y[KMAX * BMAX];       // Y[j * BMAX + r]: component j of the r-th lowest eigenvector of G(0:k,0:k)
+    double S[KMAX * BMAX];       // S[r * KMAX + j]: dot products V(:,j)^T z_r of the last bvtw pass
+    double theta[BMAX], rho2[BMAX], nx2[BMAX];
+    double gram[BMAX * BMAX], Rinv[BMAX * BMAX];
+    int error, pad[3];
+};
+
 struct Timing { bool enabled = false; cudaEvent_t ev[10]; double ms[8]; bool created = false; };
 
 struct Plan {
@@ -140,6 +154,9 @@ struct Plan {
     int *vec_counter = nullptr;
     int vec_grid = 0;
     double *Vown = nullptr, *Wown = nullptr; long long ldv_own = 0;   // dmrg_lowest_eigenpair
+    // block Davidson (allocated at plan time when options.max_rhs >= 2)
+    BlockState *bstate = nullptr, *bstate_host = nullptr;
+    double *btvec = nullptr, *bxs = nullptr, *bws = nullptr, *bpartials = nullptr; long long bld = 0;
     // stats / misc
     dmrg_stats stats{};
     long long device_bytes = 0;
@@ -147,6 +164,8 @@ struct Plan {
     std::string err;
     Timing timing;
     int sm_count = 148;
+    int max_rhs = 1;                    // right-hand sides the workspaces are sized for (options.max_rhs)
+    long long tws_elems = 0, part_elems = 0, xp_elems = 0, xq_elems = 0; int n_counters = 0;   // per right-hand side
     // dmrg_davidson_step_host: W(:,k-1) leaves on a side stream as soon as the projection is done
     cudaStream_t side = nullptr;
     cudaEvent_t ev_apply = nullptr, ev_side = nullptr;
@@ -173,7 +192,16 @@ int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s
 // Optional side job of the last CTAs of an apply: pull the first `rows` rows of `cols` columns (column stride `ld`)
 // into L2 for the kernel that follows (the Davidson basis for line 3), while the launch drains and HBM is idle.
 struct Prefetch { const double *base = nullptr; long long ld = 0, rows = 0; int cols = 0, first_ticket = 0, n_ctas = 0; };
-int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf = nullptr);
+int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf = nullptr,
+            int nrhs = 1, long long ldx = 0, long long ldy = 0);
+
+// block.cu
+int block_alloc(Plan *p);
+void block_free(Plan *p);
+int bdav_init(Plan *p, int nb, const double *X0, long long ldx0, double *V, double *W, long long ldv, cudaStream_t st);
+int bdav_step(Plan *p, double *V, double *W, long long ldv, int *k, int *na, int nb, double *theta, double *resnorm,
+              int *converged, cudaStream_t st);
+int bdav_ritz(Plan *p, const double *V, const double *W, long long ldv, int k, int nb, double *X_out, long long ldxo, cudaStream_t st);
 
 // probe.cu
 int probe_fp64(int kind, int reps, double *tflops, cudaStream_t st);

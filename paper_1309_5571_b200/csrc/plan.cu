@@ -187,6 +187,9 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     if (p->opt.max_iter <= 0) p->opt.max_iter = 2000;
     if (p->opt.reorth <= 0) p->opt.reorth = 1;
     if (p->opt.check_every <= 0) p->opt.check_every = 8;
+    if (p->opt.max_rhs <= 0) p->opt.max_rhs = 1;
+    if (p->opt.max_rhs > BMAX) { delete p; return fail(nullptr, DMRG_E_INVALID_ARG, "options: max_rhs must be 1..4"); }
+    p->max_rhs = p->opt.max_rhs;
     if (p->opt.k_max < 2 || p->opt.k_max > KMAX || p->opt.reorth > 2 || !(p->opt.tol >= 0.0)) {
         delete p; return fail(nullptr, DMRG_E_INVALID_ARG, "options: need 2 <= k_max <= 32, reorth in {1,2}, tol >= 0");
     }
@@ -555,6 +558,10 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
 
     // ---- device allocations
     CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
+    // per-apply buffers and counters exist once per right-hand side (options.max_rhs; block Davidson)
+    const int R = p->max_rhs;
+    p->tws_elems = tws_elems; p->part_elems = part_elems; p->xp_elems = xp_elems; p->xq_elems = xq_elems; p->n_counters = n_counters;
+    tws_elems *= R; part_elems *= R; xp_elems *= R; xq_elems *= R; n_counters *= R;
     CUDA_TRY(p, dev_alloc(p, &p->tws, tws_elems));
     CUDA_TRY(p, dev_alloc(p, &p->part, part_elems));
     CUDA_TRY(p, dev_alloc(p, &p->ximg_p, xp_elems));
@@ -568,11 +575,11 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
     CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
-    CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + p->n_deps));
-    CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + p->n_deps)));
+    CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + (long long)p->n_deps * R));
+    CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
     if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
         // 4 words per unit, then 4 words per CTA (phase stamps: entry, X images written, producer released, exit)
-        p->trace_units = (int)units.size() + 8 * p->sm_count;
+        p->trace_units = (int)units.size() * R + 8 * p->sm_count;
         CUDA_TRY(p, dev_alloc(p, &p->trace, 4LL * std::max<long long>(p->trace_units, 1)));
         CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     }
@@ -620,6 +627,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
     CUDA_TRY(p, gemm_kernel_setup());
     dav_setup(p);
+    { int rcb = block_alloc(p); if (rcb != DMRG_OK) { std::string m = p->err; plan_free(p); return fail(nullptr, rcb, m); } }
     CUDA_TRY(p, cudaDeviceSynchronize());
 
     // ---- stats
@@ -645,6 +653,7 @@ void plan_free(Plan *p) {
     cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
     cudaFree(p->Vown); cudaFree(p->Wown);
+    block_free(p);
     if (p->timing.created) for (auto &e : p->timing.ev) cudaEventDestroy(e);
     if (p->ev_apply) cudaEventDestroy(p->ev_apply);
     if (p->ev_side) cudaEventDestroy(p->ev_side);
