@@ -215,8 +215,11 @@ def gemv_trans_probe(plan, V, W, flush, hbm_peak):
     return out
 
 
-def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
-    """BLAS-2 kernels inside running Davidson steps at a config whose basis is far larger than L2."""
+def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36, hbm_read=None):
+    """BLAS-2 kernels inside running Davidson steps at a config whose basis is far larger than L2.  GB/s = ALGORITHMIC
+    bytes / device time; the fused residual pass re-reads V for s = V^T t out of L1/L2, so a figure above
+    the copy bandwidth is L2 assistance, not HBM traffic (profiles/r2_davidson_dram.md has the dram__bytes counters).
+    Two denominators: the read+write copy bandwidth of MEASURED_PEAKS.json and a live read-only stream probe."""
     import torch
     problem, cfg = make_problem(name)
     k_max = cfg["k_max"]
@@ -248,6 +251,10 @@ def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36):
     out["blas2_gbs"] = tot_b / (tot_ms * 1e-3) / 1e9
     out["blas2_frac_hbm"] = out["blas2_gbs"] / hbm_peak
     out["kernels_frac_hbm"] = {nm: g / hbm_peak for nm, g in out["kernels_gbs"].items()}
+    if hbm_read:
+        out["hbm_read_probe_gbs"] = hbm_read
+        out["kernels_frac_hbm_read"] = {nm: g / hbm_read for nm, g in out["kernels_gbs"].items()}
+        out["blas2_frac_hbm_read"] = out["blas2_gbs"] / hbm_read
     out["apply_tflops"] = st["flop_per_apply"] / (sum(t_apply) / len(t_apply) * 1e-3) / 1e12
     out["device_bytes"] = st["device_bytes"] + 2 * V.numel() * 8
     out["peak_allocated_bytes"] = int(torch.cuda.max_memory_allocated())
@@ -414,7 +421,8 @@ def run_ours(args):
     except Exception:
         pass
     achieved = st["flop_per_apply"] / (gemm_ms * 1e-3) / 1e12
-    roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (DMMA.8x8x4; 1 launch per step: stage-1 and stage-2 units in ticket order)",
+    roofline = {"bound": "tensor", "kernel": "grouped_gemm_kernel (persistent, warp-specialised: DMMA.8x8x4 consumers fed by cp.async.bulk tile images; "
+                                             "1 launch per step: X images, stage-1 and stage-2 units in ticket order)",
                 "achieved": achieved, "peak": max(dmma_peak, dfma_peak), "unit": "TFLOP/s",
                 "frac": achieved / max(dmma_peak, dfma_peak), "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": "measured live: register-only DMMA.8x8x4 issue-rate probe (dmrg_probe_fp64_peak); "
@@ -429,20 +437,52 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    side = world == 1 and not args.profile_run
+    gt_probe = None
     try:
-        gt_probe = gemv_trans_probe(plan, V, W, flush, hbm_peak)
+        if side:
+            gt_probe = gemv_trans_probe(plan, V, W, flush, hbm_peak)
     except Exception as e:
         gt_probe = {"error": repr(e)}
     dav_large = None
     if world == 1 and not args.no_large:
         try:
-            dav_large = davidson_hbm_probe(lib, f"cuda:{local}", hbm_peak)
+            hbm_read = lib.dmrg_probe_hbm_read(4 << 30, 3)       # live read-only stream (the BLAS-2 kernels are read-dominated)
+            dav_large = davidson_hbm_probe(lib, f"cuda:{local}", hbm_peak, hbm_read=hbm_read)
             dav_large["apply_frac_fp64_peak"] = dav_large["apply_tflops"] / max(dmma_peak, dfma_peak)
+            dav_large["other_configs"] = {}
+            for nm in ("cfg5a", "heis4096"):     # the judgement is also taken at 5a and the 4096 sweep
+                o = davidson_hbm_probe(lib, f"cuda:{local}", hbm_peak, name=nm, steps=40, hbm_read=hbm_read)
+                dav_large["other_configs"][nm] = {kk: o[kk] for kk in ("workload", "kernels_gbs", "kernels_frac_hbm", "kernels_frac_hbm_read",
+                                                                       "blas2_gbs", "blas2_frac_hbm", "blas2_frac_hbm_read") if kk in o}
         except Exception as e:   # the headline numbers above do not depend on this extra config
             dav_large = {"error": repr(e)}
+    vendor = None
+    if side:
+        try:      # the vendor-library mark beside the live probe
+            a = torch.randn(8192, 8192, dtype=torch.float64, device=f"cuda:{local}"); b = torch.randn_like(a)
+            torch.matmul(a, b); torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(3):
+                torch.matmul(a, b)
+            e1.record(stream); torch.cuda.synchronize()
+            vendor = 3 * 2.0 * 8192 ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12
+            del a, b
+            torch.cuda.empty_cache()
+        except Exception:
+            vendor = None
+    roofline["vendor_dgemm_tflops"] = vendor
+    roofline["vendor_dgemm_note"] = "torch.matmul FP64 8192^3 (cuBLAS DGEMM), 3 back-to-back calls; datasheet FP64 tensor 40 TFLOP/s nominal"
+    block = None
+    if side:
+        try:
+            block = block_davidson_probe(lib, problem, cfg, f"cuda:{local}", st)
+        except Exception as e:
+            block = {"error": repr(e)}
 
     curve = None
-    if world == 1:
+    if side:
         try:
             names = ["cfg2", "cfg4", "cfg5a", "heis4096"] + ([] if args.no_large else ["heis8192"])
             curve = hpsi_curve(lib, f"cuda:{local}", max(dmma_peak, dfma_peak), names)
@@ -481,11 +521,49 @@ def run_ours(args):
                          "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
                          "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
                          "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
-            "davidson_hbm": dav_large, "gemv_trans": gt_probe, "hpsi_curve": curve,
+            "davidson_hbm": dav_large, "gemv_trans": gt_probe, "hpsi_curve": curve, "block_davidson": block,
             "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def block_davidson_probe(lib, problem, cfg, device, st):
+    """(a) the projection of nrhs vectors in ONE grouped launch against nrhs single
+    launches; (b) the whole solve to tol 1e-10 from start (D): single-vector driver (lowest pair) vs the block driver with
+    nb = 2 (the two lowest pairs), wall clock around the C-ABI call, with the number of projections each needed."""
+    import torch
+    plan = lib.Plan(problem, k_max=cfg["k_max"], tol=1e-10, max_iter=4000, max_rhs=4, device=device)
+    n = plan.n
+    stream = torch.cuda.current_stream()
+    ld = (n + 15) // 16 * 16
+    X = torch.randn((4, ld), dtype=torch.float64, device=device); Y = torch.empty_like(X)
+    out = {"apply_multi_us_per_vector": {}}
+    for nr in (1, 2, 4):
+        for _ in range(3):
+            plan.apply_H_multi(X[:nr], Y[:nr])
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(10):
+            plan.apply_H_multi(X[:nr], Y[:nr])
+        e1.record(stream); torch.cuda.synchronize()
+        out["apply_multi_us_per_vector"][str(nr)] = e0.elapsed_time(e1) / 10 / nr * 1e3
+    out["apply_multi_tflops_nrhs4"] = st["flop_per_apply"] / (out["apply_multi_us_per_vector"]["4"] * 1e-6) / 1e12
+    D = plan.diag()
+    t0 = time.perf_counter(); rc1, lam, x, rho, it1 = plan.lowest_eigenpair(None, start_at_argmin_diag=True); torch.cuda.synchronize()
+    t_single = time.perf_counter() - t0
+    X0 = torch.zeros((2, ld), dtype=torch.float64, device=device)     # start (D) with two columns: unit vectors at the two smallest D_pp
+    idx = torch.argsort(D, stable=True)[:2]
+    X0[0, idx[0]] = 1.0; X0[1, idx[1]] = 1.0
+    t0 = time.perf_counter(); rc2, th, Xb, rb, itb, apb = plan.block_lowest_eigenpairs(X0); torch.cuda.synchronize()
+    t_block = time.perf_counter() - t0
+    out["solve"] = {"single": {"rc": rc1, "ms": t_single * 1e3, "applies": it1, "lambda": lam, "resnorm": rho},
+                    "block_nb2": {"rc": rc2, "ms": t_block * 1e3, "block_iterations": itb, "applies": apb,
+                                  "theta": [float(v) for v in th], "resnorm": [float(v) for v in rb]},
+                    "note": "block: two pairs to 1e-10, two synchronisations per block iteration (first slice); "
+                            "single: one pair, steps enqueued back to back"}
+    plan.close()
+    return out
 
 
 def hpsi_curve(lib, device, fp64_peak, names):
@@ -533,8 +611,20 @@ def main():
     ap.add_argument("--config", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-large", action="store_true", help="skip the config-5b Davidson HBM measurement")
+    ap.add_argument("--profile-run", action="store_true",
+                    help="steps only (no side probes, no CPU baseline): the command line the ncu captures under profiles/ use")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.profile_run:
+        args.no_large = args.no_cpu_baseline = True
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N replicas ourselves, the way the driver does (one rank per GPU)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

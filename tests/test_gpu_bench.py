@@ -25,7 +25,12 @@ def test_bench_line_contract():
     # 12 steps of >= 6 launches each, counted by the library
     assert d["gpu_launches"] >= 6 * 12
     rf = d["roofline"]
-    assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s" and 10.0 < rf["peak"] < 45.0      # 37 at 1.965 GHz; lower if the box runs power-capped
+    assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s"
+    # the denominator is the DMMA issue rate: 148 SMs x 128 FLOP/clk x the SM clock (37.2 TFLOP/s at 1965 MHz); it may sit
+    # below the figure for the maximum clock when the box runs power-capped, never above it
+    per_mhz = 148 * 128 * 1e6 / 1e12
+    assert 0.80 * per_mhz * d["clocks"]["sm_mhz"] <= rf["peak"] <= 1.03 * per_mhz * d["clocks"]["sm_max_mhz"]
+    assert rf["vendor_dgemm_tflops"] is None or 5.0 < rf["vendor_dgemm_tflops"] < 60.0
     assert rf["frac"] == pytest.approx(rf["achieved"] / rf["peak"]) and 0.0 < rf["frac"] < 1.0
     e = d["e2e"]
     assert 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] == 8 * 35465 and e["d2h_bytes_per_step"] == 8 * 35465 + 24
@@ -35,3 +40,6 @@ def test_bench_line_contract():
     c = d["clocks"]
     assert c["sm_max_mhz"] >= c["sm_mhz"] > 0 and isinstance(c["reasons"], list)
     assert set(d["hpsi_curve"]) >= {"cfg2", "cfg4", "cfg5a", "heis4096"}
+    b = d["block_davidson"]
+    assert "error" not in b and b["solve"]["single"]["rc"] == 0 and b["solve"]["block_nb2"]["rc"] == 0
+    assert abs(b["solve"]["single"]["lambda"] - b["solve"]["block_nb2"]["theta"][0]) <= 1e-8
