@@ -25,6 +25,15 @@
  *    its blocks, never assumed (reading A4).
  *  - FP64 throughout.  Results are run-to-run bitwise reproducible: no floating-point
  *    atomics, every reduction has a fixed order (reading A23).
+ *  - A plan serves ONE call at a time: its control words (ticket counter, ready counters),
+ *    the T workspace, the split-K partial tiles, the X tile images and the Davidson state
+ *    are per plan.  Calls on one plan must not be issued from several host threads at once.
+ *    Calls may name different streams: the library orders them itself (every hot call
+ *    records a plan-owned event, and a call on another stream first waits for it), so two
+ *    applies of one plan never overlap on the device.  Use one plan per concurrent solve.
+ *  - If a dependency wait inside the projection kernel ever gives up (seconds; a lost or
+ *    foreign launch), a sticky error word is set and the next synchronising call returns
+ *    DMRG_E_CUDA instead of hanging the stream.
  */
 #ifndef DMRG_B200_H
 #define DMRG_B200_H
@@ -96,6 +105,8 @@ typedef struct {
     int32_t  tile;      /* projection tile selector: 0 = auto                            */
     int32_t  check_every; /* dmrg_lowest_eigenpair: host reads the device convergence flag
                              every this many iterations (0 = default 8)                   */
+    int32_t  reserve_basis; /* != 0: allocate the drivers' own V, W at plan creation, so that
+                               dmrg_lowest_eigenpair / dmrg_block_lowest_eigenpairs allocate nothing */
     int32_t  max_rhs;     /* largest number of vectors one projection launch takes
                              (dmrg_apply_H_multi, block Davidson): 1..4, 0 = 1.  The per-apply
                              workspaces are allocated max_rhs times at plan creation.       */
@@ -109,7 +120,8 @@ typedef struct {
     int64_t flop_per_apply;    /* algorithmic FLOP, reading A24                           */
     int64_t operator_elems;    /* operator-block elements the apply reads (unpadded)      */
     int64_t apply_bytes;       /* 8*(operator_elems + 2n): compulsory traffic per apply   */
-    int32_t stage1_units, stage2_units; /* CTAs of the two grouped launches               */
+    int32_t stage1_units, stage2_units; /* work units (64x64 tile x K slice) of the two GEMM
+                                           stages; one persistent launch runs both          */
     int32_t stage2_split_tiles;/* output tiles whose concatenated K is split              */
     int64_t pool_bytes;        /* repacked operator pool                                  */
     int64_t workspace_bytes;   /* T + split-K partials + Davidson scratch                 */
@@ -129,7 +141,7 @@ typedef struct dmrg_plan *dmrg_handle_t;
  * are fixed"): admissible pairs, operation records grouped by output segment (L342, L358:
  * "all records of the same output on the same [owner]" -> atomics-free accumulation),
  * per-record association order by FLOP (A24), the repacked operator pool (scaled,
- * transposed, 16-byte aligned rows), work units for the two grouped launches, diag(H_SB)
+ * transposed, stored as 8 KB tile images), the work units of the grouped launch, diag(H_SB)
  * (A14) and all workspaces.  Reads the operator data on the device (stream NULL) and
  * synchronises before returning.  opts may be NULL (k_max 20, tol 1e-10, max_iter 2000,
  * reorth 1).  On failure *out = NULL and dmrg_last_error(NULL) has the reason. */
@@ -210,7 +222,8 @@ int dmrg_ritz_vector(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
 /* Driver (Alg. 3 looped): lowest eigenpair of H_SB on the target sector.
  * x0 DEVICE or NULL (seeded start; start_at_argmin_diag as in dmrg_davidson_init);
  * x_out DEVICE n doubles (normalised Ritz vector); lambda, resnorm, iters HOST.
- * Uses plan-owned V, W (allocated on first use: 2 * n * k_max doubles).  The convergence
+ * Uses plan-owned V, W (2 * n * k_max doubles: allocated at plan creation with
+ * options.reserve_basis != 0, else on the first call of a driver).  The convergence
  * test runs on the device; the host polls it every options.check_every iterations, so up
  * to check_every-1 no-op launches may follow convergence; the reported iteration count is
  * the exact one.  Returns DMRG_OK, DMRG_NOT_CONVERGED or an error. */
@@ -277,7 +290,9 @@ int dmrg_get_timing(dmrg_handle_t h, double *ms8);
 /* Diagnostics: per-work-unit timeline of the LAST dmrg_apply_H of this plan, recorded only when the
  * plan was created with the environment variable DMRG_TRACE set (otherwise *n_units = 0).
  * trace_host: HOST array of 4 * max_units uint64 -- per unit, in issue (ticket) order:
- * start ns, end-of-main-loop ns, end ns (%globaltimer), SM id.  Synchronises the device. */
+ * start ns, end-of-main-loop ns, end ns (%globaltimer), packed word (bits 0-15 SM id, 16-31
+ * k-tiles, 32-47 CTA, 48 stage-1 unit, 49 split-K unit, 50 wrote C); after the units, one
+ * row per CTA: kernel entry, X images written, producer released, exit.  Synchronises the device. */
 int dmrg_get_unit_trace(dmrg_handle_t h, uint64_t *trace_host, int32_t max_units, int32_t *n_units);
 
 int dmrg_version(void);

@@ -56,7 +56,8 @@ class _Problem(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("tol", C.c_double), ("max_iter", C.c_int32), ("reorth", C.c_int32),
-                ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32), ("max_rhs", C.c_int32)]
+                ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32), ("reserve_basis", C.c_int32),
+                ("max_rhs", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -154,7 +155,7 @@ class Plan:
     """Owns a dmrg_handle_t plus the device copies of the operator blocks."""
 
     def __init__(self, problem, k_max: int = 20, tol: float = 1e-10, max_iter: int = 2000, reorth: int = 1,
-                 seed: int = 1, check_every: int = 8, max_rhs: int = 1, device: Optional[str] = None):
+                 seed: int = 1, check_every: int = 8, max_rhs: int = 1, reserve_basis: bool = False, device: Optional[str] = None):
         torch = _torch()
         self._lib = load_library()
         self._keep = []
@@ -171,7 +172,7 @@ class Plan:
         tgt = np.ascontiguousarray(np.asarray(problem.target, dtype=np.int32).ravel())
         self._keep.append(tgt)
         pr.target = tgt.ctypes.data_as(C.POINTER(C.c_int32))
-        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(max_rhs))
+        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(bool(reserve_basis)), int(max_rhs))
         h = C.c_void_p()
         rc = self._lib.dmrg_plan_create(C.byref(pr), C.byref(opt), C.byref(h))
         if rc != DMRG_OK:

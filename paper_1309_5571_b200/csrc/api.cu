@@ -89,7 +89,10 @@ int dmrg_apply_H(dmrg_handle_t h, const double *x, double *y, void *stream) {
     Plan *p = P(h);
     if (!x || !y) return fail(p, DMRG_E_INVALID_ARG, "apply_H: NULL vector");
     if ((x <= y && y < x + p->n) || (y <= x && x < y + p->n)) return fail(p, DMRG_E_INVALID_ARG, "apply_H: x and y overlap");
-    return apply_H(p, x, y, nullptr, S(stream));
+    stream_enter(p, S(stream));
+    const int rc = apply_H(p, x, y, nullptr, S(stream));
+    stream_leave(p, S(stream));
+    return rc;
 }
 
 int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmin_diag, double *V, double *W,
@@ -97,14 +100,20 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
     if (!h) return DMRG_E_INVALID_ARG;
     Plan *p = P(h);
     if (!V || !W || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "davidson_init: NULL basis or ldv < n");
-    return dav_init(p, x0, start_at_argmin_diag, V, W, ldv, S(stream));
+    p->state_host->done = 0;
+    stream_enter(p, S(stream));
+    const int rc = dav_init(p, x0, start_at_argmin_diag, V, W, ldv, S(stream));
+    stream_leave(p, S(stream));
+    return rc;
 }
 
 static int step_common(Plan *p, double *V, double *W, int64_t ldv, int32_t *k, double *lambda, double *resnorm,
                        int32_t *converged, cudaStream_t st, bool enqueue_only) {
     if (p->timing.enabled) ensure_timing(p);
     int k_next = *k;
+    stream_enter(p, st);
     int rc = dav_enqueue_step(p, V, W, ldv, *k, st, &k_next);
+    stream_leave(p, st);
     if (rc != DMRG_OK) return rc;
     if (enqueue_only) {   // no stream synchronisation (see dmrg_davidson_poll)
         *k = k_next;
@@ -143,13 +152,8 @@ int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, 
     if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_host: NULL argument");
     if (*k < 1 || *k > p->opt.k_max || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_host: k or ldv out of range");
     cudaStream_t st = S(stream);
-    if (w_out_host && !p->side) {
-        cudaError_t e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_apply, cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
-        if (e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));
-    }
-    if (v_in_host)
+    // a run that has already converged makes the step a no-op: do not overwrite a column dmrg_ritz_vector still needs
+    if (v_in_host && p->state_host->done != 1)
         cudaMemcpyAsync(V + (long long)(*k - 1) * ldv, v_in_host, sizeof(double) * p->n, cudaMemcpyHostToDevice, st);
     p->w_out_host = w_out_host;
     int rc = step_common(p, V, W, ldv, k, lambda, resnorm, converged, st, false);
@@ -271,7 +275,10 @@ int dmrg_apply_H_multi(dmrg_handle_t h, int32_t nrhs, const double *x, int64_t l
     if (!x || !y || ldx < p->n || ldy < p->n) return fail(p, DMRG_E_INVALID_ARG, "apply_H_multi: NULL vectors or a column stride below n");
     const double *xe = x + (nrhs - 1) * ldx + p->n; const double *ye = y + (nrhs - 1) * ldy + p->n;
     if (!(xe <= y || ye <= x)) return fail(p, DMRG_E_INVALID_ARG, "apply_H_multi: x and y overlap");
-    return apply_H(p, x, y, nullptr, S(stream), nullptr, nrhs, ldx, ldy);
+    stream_enter(p, S(stream));
+    const int rc = apply_H(p, x, y, nullptr, S(stream), nullptr, nrhs, ldx, ldy);
+    stream_leave(p, S(stream));
+    return rc;
 }
 
 int dmrg_block_init(dmrg_handle_t h, int32_t nb, const double *X0, int64_t ldx0, double *V, double *W, int64_t ldv, void *stream) {
@@ -285,7 +292,9 @@ int dmrg_block_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t 
     Plan *p = P(h);
     if (!V || !W || !k || !na) return fail(p, DMRG_E_INVALID_ARG, "block_step: NULL argument");
     int kk = *k, nn = *na;
+    stream_enter(p, S(stream));
     int rc = bdav_step(p, V, W, ldv, &kk, &nn, nb, theta, resnorm, converged, S(stream));
+    stream_leave(p, S(stream));
     if (rc == DMRG_OK) { *k = kk; *na = nn; }
     return rc;
 }

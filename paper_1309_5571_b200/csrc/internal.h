@@ -169,6 +169,8 @@ struct Plan {
     // dmrg_davidson_step_host: W(:,k-1) leaves on a side stream as soon as the projection is done
     cudaStream_t side = nullptr;
     cudaEvent_t ev_apply = nullptr, ev_side = nullptr;
+    // one call at a time: a hot call on another stream than the previous one first waits for this event
+    cudaEvent_t ev_last = nullptr; cudaStream_t last_stream = nullptr; bool last_valid = false;
     double *w_out_host = nullptr;       // non-null only while such a step is being enqueued
 };
 
@@ -178,6 +180,10 @@ int fail(Plan *p, int code, const std::string &msg);
 // plan.cu
 int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out);
 void plan_free(Plan *p);
+
+// plan.cu: ordering of hot calls of one plan across streams (include/dmrg_b200.h "A plan serves ONE call at a time")
+void stream_enter(Plan *p, cudaStream_t st);
+void stream_leave(Plan *p, cudaStream_t st);
 
 // gemm.cu
 cudaError_t gemm_kernel_setup();

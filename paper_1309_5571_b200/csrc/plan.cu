@@ -27,6 +27,13 @@ int fail(Plan *p, int code, const std::string &msg) {
     return code;
 }
 
+void stream_enter(Plan *p, cudaStream_t st) {
+    if (p->last_valid && p->last_stream != st) cudaStreamWaitEvent(st, p->ev_last, 0);
+}
+void stream_leave(Plan *p, cudaStream_t st) {
+    if (p->ev_last) { cudaEventRecord(p->ev_last, st); p->last_stream = st; p->last_valid = true; }
+}
+
 // ---------------------------------------------------------------- plan-time kernels
 __global__ void repack_kernel(RepackJob j, double *pool) {
     __shared__ double tile[32][33];
@@ -627,6 +634,17 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
     CUDA_TRY(p, gemm_kernel_setup());
     dav_setup(p);
+    // everything a hot call needs exists from here on: side stream and events of dmrg_davidson_step_host, the ordering
+    // event, and (options.reserve_basis) the drivers' own basis
+    CUDA_TRY(p, cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking));
+    CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_apply, cudaEventDisableTiming));
+    CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming));
+    CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_last, cudaEventDisableTiming));
+    if (p->opt.reserve_basis) {
+        p->ldv_own = (p->n + 15) / 16 * 16;
+        CUDA_TRY(p, dev_alloc(p, &p->Vown, p->ldv_own * p->opt.k_max));
+        CUDA_TRY(p, dev_alloc(p, &p->Wown, p->ldv_own * p->opt.k_max));
+    }
     { int rcb = block_alloc(p); if (rcb != DMRG_OK) { std::string m = p->err; plan_free(p); return fail(nullptr, rcb, m); } }
     CUDA_TRY(p, cudaDeviceSynchronize());
 
@@ -657,6 +675,7 @@ void plan_free(Plan *p) {
     if (p->timing.created) for (auto &e : p->timing.ev) cudaEventDestroy(e);
     if (p->ev_apply) cudaEventDestroy(p->ev_apply);
     if (p->ev_side) cudaEventDestroy(p->ev_side);
+    if (p->ev_last) cudaEventDestroy(p->ev_last);
     if (p->side) cudaStreamDestroy(p->side);
     delete p;
 }

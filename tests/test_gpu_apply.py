@@ -249,3 +249,37 @@ def test_apply_matches_oracle_fuzz(lib, seed, monkeypatch):
         assert torch.equal(y, y2)
         assert rel_maxnorm(y.cpu().numpy(), want) <= HPSI_RTOL, (seed, ups)
         plan.close()
+
+
+def test_two_streams_on_one_plan_are_ordered(lib):
+    """include/dmrg_b200.h: a plan serves one call at a time; calls that name different streams are ordered by the library
+    (plan-owned event).  Applies of ONE plan issued alternately on two streams, without any synchronisation by the
+    caller, must give the bits of the single-stream results (interleaved tickets would give garbage or hang)."""
+    import torch
+    p = full_config("cfg2")
+    lay = rec.Layout(p)
+    plan = lib.Plan(p, k_max=4)
+    xs = [to_dev(random_vector(lay.n, 700 + i)) for i in range(6)]
+    ref = [plan.apply_H(x).clone() for x in xs]
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = [torch.empty_like(x) for x in xs]
+    for rep in range(5):
+        for i, x in enumerate(xs):
+            plan.apply_H(x, outs[i], stream=(s1 if i % 2 == 0 else s2))
+    torch.cuda.synchronize()
+    for o, r in zip(outs, ref):
+        assert torch.equal(o, r)
+    plan.close()
+
+
+def test_reserved_basis_driver_allocates_nothing(lib):
+    """options.reserve_basis: the driver's V, W exist after plan creation (no allocation in the hot calls)."""
+    import torch
+    p = SMALL["cfg2_m160"]()
+    plan = lib.Plan(p, k_max=12, tol=1e-9, reserve_basis=True)
+    b0 = plan.stats()["device_bytes"]
+    assert b0 >= 2 * 8 * plan.n * 12
+    rc, lam, x, rho, iters = plan.lowest_eigenpair(None, start_at_argmin_diag=True)
+    assert rc == lib.DMRG_OK and plan.stats()["device_bytes"] == b0
+    plan.close()
