@@ -2,7 +2,9 @@
 // Not part of the ABI (include/dmrg_b200.h is).
 #pragma once
 #include <cstdint>
+#include <map>
 #include <string>
+#include <tuple>
 #include <vector>
 #include <cuda_runtime.h>
 #include "../../include/dmrg_b200.h"
@@ -169,6 +171,10 @@ struct Plan {
     // dmrg_davidson_step_host: W(:,k-1) leaves on a side stream as soon as the projection is done
     cudaStream_t side = nullptr;
     cudaEvent_t ev_apply = nullptr, ev_side = nullptr;
+    // CUDA graphs of dmrg_davidson_step, one per (V, W, ldv, basis size)
+    typedef std::tuple<const void *, const void *, long long, int> GraphKey;
+    struct GraphEntry { cudaGraphExec_t exec; int k_next; int launches; };
+    std::map<GraphKey, GraphEntry> graphs;
     // one call at a time: a hot call on another stream than the previous one first waits for this event
     cudaEvent_t ev_last = nullptr; cudaStream_t last_stream = nullptr; bool last_valid = false;
     double *w_out_host = nullptr;       // non-null only while such a step is being enqueued

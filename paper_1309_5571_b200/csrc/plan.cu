@@ -676,6 +676,7 @@ void plan_free(Plan *p) {
     if (p->ev_apply) cudaEventDestroy(p->ev_apply);
     if (p->ev_side) cudaEventDestroy(p->ev_side);
     if (p->ev_last) cudaEventDestroy(p->ev_last);
+    for (auto &g : p->graphs) cudaGraphExecDestroy(g.second.exec);
     if (p->side) cudaStreamDestroy(p->side);
     delete p;
 }
