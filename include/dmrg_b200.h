@@ -263,6 +263,45 @@ int dmrg_block_lowest_eigenpairs(dmrg_handle_t h, int32_t nb, const double *X0, 
                                  int64_t ldxo, double *theta, double *resnorm, int32_t *iters, int32_t *applies,
                                  void *cuda_stream);
 
+/* ---- the steps either side of the path: Alg. 1 lines 2, 5-7 ---- */
+
+/* Line 5: reduced density matrix of one side of the plan's superblock from a target-sector vector x (DEVICE, n doubles,
+ * normalised or not): side 0 = left, rho_i = sum_k X_ik X_ik^T; side 1 = right, rho_k = sum_i X_ik^T X_ik.
+ * rho_out DEVICE: the sectors of that side in index order, each row-major d_s x d_s, back to back (sum_s d_s^2 doubles;
+ * zero matrix for a sector without a pair).  Synchronises the stream. */
+int dmrg_density_matrix(dmrg_handle_t h, const double *x, int32_t side, double *rho_out, void *cuda_stream);
+/* Line 6: all eigenpairs of n_sectors symmetric blocks (layout as rho_out; rho is destroyed): U_out (same layout, columns =
+ * eigenvectors by DESCENDING eigenvalue), w_out DEVICE (sum_s d_s doubles, descending per sector).  dims HOST. */
+int dmrg_sector_eig(int32_t n_sectors, const int32_t *dims, double *rho, double *U_out, double *w_out, void *cuda_stream);
+/* Line 7, the choice (host only): the m largest eigenvalues over all sectors (ties: lower sector index, then higher rank
+ * inside the sector; eigenvalues <= 0 are never kept).  w_host as w_out; m_keep HOST [n_sectors] out; *discarded = sum of
+ * all eigenvalues - sum of the kept ones. */
+int dmrg_select_states(int32_t n_sectors, const int32_t *dims, const double *w_host, int32_t m, int32_t *m_keep,
+                       double *discarded);
+/* Line 7, the rotation: for every block b of `op` (index arrays HOST, data DEVICE), O'_b = U_dst(:, 0:m_dst)^T A_b
+ * U_src(:, 0:m_src).  out_data DEVICE: the rotated blocks back to back, row-major m_dst x m_src (NULL: sizes only);
+ * out_offset HOST [n_blocks]: element offset of each, -1 for a block that disappears; *out_elems: doubles needed. */
+int dmrg_rotate_op(int32_t n_sectors, const int32_t *dims, const int32_t *m_keep, const double *U, const dmrg_block_op *op,
+                   double *out_data, int64_t *out_offset, int64_t *out_elems, void *cuda_stream);
+
+/* Alg. 1 looped (infinite-lattice algorithm) for the open spin-1/2 Heisenberg chain: from two single-site blocks,
+ * every iteration enlarges both blocks by one site (line 2), finds the ground state of the LR superblock in the S_z = 0
+ * sector with dmrg_lowest_eigenpair (line 3, start e_argmin(D)), builds both density matrices (5), diagonalises them (6) and
+ * keeps the m_keep states of largest weight (7), until the superblock has n_sites sites.  One record per iteration (HOST
+ * arrays of max_records; any may be NULL): superblock sites, ground-state energy, discarded weights, target-sector
+ * dimension, Davidson iterations. */
+typedef struct {
+    int32_t n_sites;   /* even, >= 4 */
+    int32_t m_keep;    /* block states kept after each iteration (the paper's m) */
+    double  J, Delta;
+    double  tol;       /* Davidson ||r|| <= tol (0 = 1e-10) */
+    int32_t k_max;     /* Davidson basis limit (0 = 20) */
+    int32_t max_iter;  /* Davidson applies per superblock (0 = 4000) */
+} dmrg_idmrg_options;
+int dmrg_infinite_heisenberg(const dmrg_idmrg_options *opts, int32_t max_records, int32_t *n_records, int32_t *n_sites,
+                             double *energy, double *discarded_left, double *discarded_right, int64_t *target_dim,
+                             int32_t *davidson_iters, void *cuda_stream);
+
 /* ---- the Davidson BLAS-2 kernels on their own (Alg. 3 lines 3, 5-6, 12-13; Alg. 4) --- */
 
 /* out[0..k) = V(:,0..k)^T w   (gemv_trans).  out DEVICE k doubles. */

@@ -26,6 +26,7 @@ EXPORTS = [
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
     "dmrg_apply_H_multi", "dmrg_block_init", "dmrg_block_step", "dmrg_block_ritz", "dmrg_block_get_small",
     "dmrg_block_lowest_eigenpairs",
+    "dmrg_density_matrix", "dmrg_sector_eig", "dmrg_select_states", "dmrg_rotate_op", "dmrg_infinite_heisenberg",
 ]
 
 
@@ -38,6 +39,11 @@ class DmrgError(RuntimeError):
 class _Sectors(C.Structure):
     _fields_ = [("n_labels", C.c_int32), ("n_sectors", C.c_int32),
                 ("labels", C.POINTER(C.c_int32)), ("dims", C.POINTER(C.c_int32))]
+
+
+class _IdmrgOptions(C.Structure):
+    _fields_ = [("n_sites", C.c_int32), ("m_keep", C.c_int32), ("J", C.c_double), ("Delta", C.c_double), ("tol", C.c_double),
+                ("k_max", C.c_int32), ("max_iter", C.c_int32)]
 
 
 class _BlockOp(C.Structure):
@@ -115,6 +121,11 @@ def load_library():
         "dmrg_block_ritz": [vp, vp, vp, i64, i32, i32, vp, i64, vp],
         "dmrg_block_get_small": [vp, i32, pdbl, pdbl, vp],
         "dmrg_block_lowest_eigenpairs": [vp, i32, vp, i64, vp, i64, pdbl, pdbl, pi32, pi32, vp],
+        "dmrg_density_matrix": [vp, vp, i32, vp, vp],
+        "dmrg_sector_eig": [i32, pi32, vp, vp, vp, vp],
+        "dmrg_select_states": [i32, pi32, pdbl, i32, pi32, pdbl],
+        "dmrg_rotate_op": [i32, pi32, pi32, vp, C.POINTER(_BlockOp), vp, pi64, pi64, vp],
+        "dmrg_infinite_heisenberg": [C.POINTER(_IdmrgOptions), i32, pi32, pi32, pdbl, pdbl, pdbl, pi64, pi32, vp],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -124,6 +135,47 @@ def load_library():
     lib.dmrg_last_error.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+def sector_eig(dims, rho, stream=None):
+    """All eigenpairs of the sector blocks in `rho` (flat CUDA tensor, destroyed): (U flat, w flat), descending per sector."""
+    torch = _torch()
+    lib = load_library()
+    d = np.ascontiguousarray(np.asarray(dims, dtype=np.int32))
+    U = torch.empty_like(rho)
+    w = torch.empty(max(int(d.sum()), 1), dtype=torch.float64, device=rho.device)
+    rc = lib.dmrg_sector_eig(len(d), d.ctypes.data_as(C.POINTER(C.c_int32)), _ptr(rho), _ptr(U), _ptr(w), _stream_ptr(stream))
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return U, w[:int(d.sum())]
+
+
+def select_states(dims, w_host, m: int):
+    """-> (m_keep per sector, discarded weight)"""
+    lib = load_library()
+    d = np.ascontiguousarray(np.asarray(dims, dtype=np.int32)); w = np.ascontiguousarray(np.asarray(w_host, dtype=np.float64))
+    mk = np.zeros(len(d), dtype=np.int32); disc = C.c_double()
+    rc = lib.dmrg_select_states(len(d), d.ctypes.data_as(C.POINTER(C.c_int32)), w.ctypes.data_as(C.POINTER(C.c_double)), int(m),
+                                mk.ctypes.data_as(C.POINTER(C.c_int32)), C.byref(disc))
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return mk, float(disc.value)
+
+
+def infinite_heisenberg(n_sites: int, m_keep: int, J: float = 1.0, Delta: float = 1.0, tol: float = 1e-10, k_max: int = 20,
+                        max_iter: int = 4000, stream=None):
+    """dmrg_infinite_heisenberg: list of dicts(n_sites, energy, discarded, n, davidson_iters), one per DMRG iteration."""
+    _torch()
+    lib = load_library()
+    cap = n_sites // 2
+    o = _IdmrgOptions(int(n_sites), int(m_keep), float(J), float(Delta), float(tol), int(k_max), int(max_iter))
+    nr = C.c_int32(); ns = (C.c_int32 * cap)(); e = (C.c_double * cap)(); dl = (C.c_double * cap)(); dr = (C.c_double * cap)()
+    td = (C.c_int64 * cap)(); it = (C.c_int32 * cap)()
+    rc = lib.dmrg_infinite_heisenberg(C.byref(o), cap, C.byref(nr), ns, e, dl, dr, td, it, _stream_ptr(stream))
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return [dict(n_sites=int(ns[q]), energy=float(e[q]), discarded=(float(dl[q]), float(dr[q])), n=int(td[q]), davidson_iters=int(it[q]))
+            for q in range(nr.value)]
 
 
 def _torch():
@@ -305,6 +357,28 @@ class Plan:
         if rc < 0:
             self._check(rc)
         return rc, np.array(th[:]), X[:, :self.n], np.array(rho[:]), int(it.value), int(ap.value)
+
+    # ---- the steps either side of the path (Alg. 1 lines 5-7)
+    def density_matrix(self, x, side: int, dims, stream=None):
+        """rho of side 0 (left) / 1 (right): flat CUDA tensor, sector s at offset sum_{t<s} d_t^2, row-major d_s x d_s."""
+        torch = _torch()
+        _check_vec(x, self.n, "x")
+        tot = int(sum(int(d) * int(d) for d in dims))
+        rho = torch.empty(max(tot, 1), dtype=torch.float64, device=self.device)
+        self._check(self._lib.dmrg_density_matrix(self._h, _ptr(x), int(side), _ptr(rho), _stream_ptr(stream)))
+        return rho[:tot]
+
+    def rotate_op(self, op, dims, m_keep, U, stream=None):
+        """-> (out_data CUDA tensor, out_offset np.int64 [n_blocks]) for a dmrg_inputs BlockOp."""
+        torch = _torch()
+        bo = self._block_op(op)
+        d = np.ascontiguousarray(np.asarray(dims, dtype=np.int32)); mk = np.ascontiguousarray(np.asarray(m_keep, dtype=np.int32))
+        off = np.zeros(max(len(op.blocks), 1), dtype=np.int64); ne = C.c_int64()
+        args = (len(d), d.ctypes.data_as(C.POINTER(C.c_int32)), mk.ctypes.data_as(C.POINTER(C.c_int32)), _ptr(U), C.byref(bo))
+        self._check(self._lib.dmrg_rotate_op(*args, None, off.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(ne), _stream_ptr(stream)))
+        out = torch.empty(max(int(ne.value), 1), dtype=torch.float64, device=self.device)
+        self._check(self._lib.dmrg_rotate_op(*args, _ptr(out), off.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(ne), _stream_ptr(stream)))
+        return out[:int(ne.value)], off[:len(op.blocks)]
 
     def _check_basis(self, V, W):
         """a wrong-shaped basis must not reach the kernels (they would write out of bounds)."""

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdmrg_b200.so")
-SOURCES = ["plan.cu", "gemm.cu", "davidson.cu", "block.cu", "probe.cu", "api.cu"]
+SOURCES = ["plan.cu", "gemm.cu", "davidson.cu", "block.cu", "renorm.cu", "probe.cu", "api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
