@@ -107,6 +107,9 @@ typedef struct {
                              every this many iterations (0 = default 8)                   */
     int32_t  reserve_basis; /* != 0: allocate the drivers' own V, W at plan creation, so that
                                dmrg_lowest_eigenpair / dmrg_block_lowest_eigenpairs allocate nothing */
+    int32_t  shard_rank, shard_count; /* output sharding over several GPUs: with
+                             shard_count > 1 the plan projects only the output segments owned by shard_rank
+                             (dmrg_get_shard); the other segments of y are left untouched.  0 = no sharding. */
     int32_t  max_rhs;     /* largest number of vectors one projection launch takes
                              (dmrg_apply_H_multi, block Davidson): 1..4, 0 = 1.  The per-apply
                              workspaces are allocated max_rhs times at plan creation.       */
@@ -153,6 +156,12 @@ int dmrg_plan_destroy(dmrg_handle_t h);
 int dmrg_get_layout(dmrg_handle_t h, int64_t *n, int32_t *n_pairs,
                     int32_t *left_sector, int32_t *right_sector, int64_t *seg_offset);
 int dmrg_get_stats(dmrg_handle_t h, dmrg_stats *stats);
+/* Output sharding ("all records of the same output on the same device", L362 workload per
+ * output): longest-processing-time assignment of n_outputs outputs with the given costs to n_ranks ranks (descending cost,
+ * ties by lower index; least loaded rank, ties by lower rank).  Host only, no device needed; every rank computes the same
+ * table.  dmrg_get_shard reports the table a plan used: owner HOST [n_pairs] (all 0 without sharding). */
+int dmrg_partition_outputs(int32_t n_outputs, const int64_t *cost, int32_t n_ranks, int32_t *owner);
+int dmrg_get_shard(dmrg_handle_t h, int32_t *owner);
 /* diag(H_SB) on the target sector (reading A14) copied to a DEVICE array of n doubles. */
 int dmrg_get_diag(dmrg_handle_t h, double *d_out, void *cuda_stream);
 const char *dmrg_last_error(dmrg_handle_t h);
@@ -188,6 +197,12 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
  * leaves V, W, B and the reported state untouched; read the state with dmrg_davidson_poll. */
 int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k,
                        double *lambda, double *resnorm, int32_t *converged, void *cuda_stream);
+
+/* dmrg_davidson_step without its line 2: W(:,k-1) = H_SB V(:,k-1) has been formed by the caller -- e.g. summed over the
+ * ranks of an output-sharded projection (each rank applies its own plan to V(:,k-1), then one all-reduce) -- and lines 3-14
+ * run as usual.  Same arguments and conventions as dmrg_davidson_step. */
+int dmrg_davidson_step_given_w(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, double *lambda,
+                               double *resnorm, int32_t *converged, void *cuda_stream);
 
 /* dmrg_davidson_step for a caller that keeps (part of) the basis on the HOST -- the setting of the
  * paper's hybrid code, where each new basis vector is uploaded and H_SB x downloaded every

@@ -26,6 +26,7 @@ EXPORTS = [
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
     "dmrg_apply_H_multi", "dmrg_block_init", "dmrg_block_step", "dmrg_block_ritz", "dmrg_block_get_small",
     "dmrg_block_lowest_eigenpairs",
+    "dmrg_partition_outputs", "dmrg_get_shard", "dmrg_davidson_step_given_w",
     "dmrg_density_matrix", "dmrg_sector_eig", "dmrg_select_states", "dmrg_rotate_op", "dmrg_infinite_heisenberg",
 ]
 
@@ -63,7 +64,7 @@ class _Problem(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("tol", C.c_double), ("max_iter", C.c_int32), ("reorth", C.c_int32),
                 ("seed", C.c_uint64), ("tile", C.c_int32), ("check_every", C.c_int32), ("reserve_basis", C.c_int32),
-                ("max_rhs", C.c_int32)]
+                ("shard_rank", C.c_int32), ("shard_count", C.c_int32), ("max_rhs", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -121,6 +122,9 @@ def load_library():
         "dmrg_block_ritz": [vp, vp, vp, i64, i32, i32, vp, i64, vp],
         "dmrg_block_get_small": [vp, i32, pdbl, pdbl, vp],
         "dmrg_block_lowest_eigenpairs": [vp, i32, vp, i64, vp, i64, pdbl, pdbl, pi32, pi32, vp],
+        "dmrg_partition_outputs": [i32, pi64, i32, pi32],
+        "dmrg_get_shard": [vp, pi32],
+        "dmrg_davidson_step_given_w": [vp, vp, vp, i64, pi32, pdbl, pdbl, pi32, vp],
         "dmrg_density_matrix": [vp, vp, i32, vp, vp],
         "dmrg_sector_eig": [i32, pi32, vp, vp, vp, vp],
         "dmrg_select_states": [i32, pi32, pdbl, i32, pi32, pdbl],
@@ -135,6 +139,17 @@ def load_library():
     lib.dmrg_last_error.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+def partition_outputs(cost, n_ranks: int):
+    """dmrg_partition_outputs: LPT owner table (host only; works without a GPU)."""
+    lib = load_library()
+    c = np.ascontiguousarray(np.asarray(cost, dtype=np.int64))
+    own = np.zeros(len(c), dtype=np.int32)
+    rc = lib.dmrg_partition_outputs(len(c), c.ctypes.data_as(C.POINTER(C.c_int64)), int(n_ranks), own.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return own
 
 
 def sector_eig(dims, rho, stream=None):
@@ -207,7 +222,8 @@ class Plan:
     """Owns a dmrg_handle_t plus the device copies of the operator blocks."""
 
     def __init__(self, problem, k_max: int = 20, tol: float = 1e-10, max_iter: int = 2000, reorth: int = 1,
-                 seed: int = 1, check_every: int = 8, max_rhs: int = 1, reserve_basis: bool = False, device: Optional[str] = None):
+                 seed: int = 1, check_every: int = 8, max_rhs: int = 1, reserve_basis: bool = False, shard_rank: int = 0, shard_count: int = 0,
+                 device: Optional[str] = None):
         torch = _torch()
         self._lib = load_library()
         self._keep = []
@@ -224,7 +240,7 @@ class Plan:
         tgt = np.ascontiguousarray(np.asarray(problem.target, dtype=np.int32).ravel())
         self._keep.append(tgt)
         pr.target = tgt.ctypes.data_as(C.POINTER(C.c_int32))
-        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(bool(reserve_basis)), int(max_rhs))
+        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(bool(reserve_basis)), int(shard_rank), int(shard_count), int(max_rhs))
         h = C.c_void_p()
         rc = self._lib.dmrg_plan_create(C.byref(pr), C.byref(opt), C.byref(h))
         if rc != DMRG_OK:
@@ -413,6 +429,19 @@ class Plan:
         self._check(self._lib.dmrg_davidson_step(self._h, _ptr(V), _ptr(W), int(ldv), C.byref(kk), None, None, None,
                                                  _stream_ptr(stream)))
         return int(kk.value)
+
+    def davidson_step_given_w(self, V, W, k: int, stream=None) -> Tuple[int, float, float, bool]:
+        """Lines 3-14 of Alg. 3 with W(:,k-1) already formed by the caller (output-sharded projection + all-reduce)."""
+        self._check_basis(V, W)
+        kk = C.c_int32(int(k)); lam = C.c_double(); rho = C.c_double(); conv = C.c_int32()
+        self._check(self._lib.dmrg_davidson_step_given_w(self._h, _ptr(V), _ptr(W), int(V.stride(0)), C.byref(kk), C.byref(lam),
+                                                         C.byref(rho), C.byref(conv), _stream_ptr(stream)))
+        return int(kk.value), float(lam.value), float(rho.value), bool(conv.value)
+
+    def shard_owner(self):
+        own = np.zeros(self.n_pairs, dtype=np.int32)
+        self._check(self._lib.dmrg_get_shard(self._h, own.ctypes.data_as(C.POINTER(C.c_int32))))
+        return own
 
     def davidson_poll(self, stream=None) -> Tuple[float, float, bool, int]:
         """(lambda, rho, converged, executed iterations) after a stream synchronisation."""

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstddef>
 #include <cstring>
+#include <vector>
 #include "internal.h"
 
 namespace dmrg { const std::string &global_error(); }
@@ -108,11 +109,11 @@ int dmrg_davidson_init(dmrg_handle_t h, const double *x0, int32_t start_at_argmi
 }
 
 static int step_common(Plan *p, double *V, double *W, int64_t ldv, int32_t *k, double *lambda, double *resnorm,
-                       int32_t *converged, cudaStream_t st, bool enqueue_only) {
+                       int32_t *converged, cudaStream_t st, bool enqueue_only, bool skip_apply = false) {
     if (p->timing.enabled) ensure_timing(p);
     int k_next = *k;
     stream_enter(p, st);
-    int rc = dav_enqueue_step(p, V, W, ldv, *k, st, &k_next);
+    int rc = dav_enqueue_step(p, V, W, ldv, *k, st, &k_next, skip_apply);
     stream_leave(p, st);
     if (rc != DMRG_OK) return rc;
     if (enqueue_only) {   // no stream synchronisation (see dmrg_davidson_poll)
@@ -143,6 +144,28 @@ int dmrg_davidson_step(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32
     Plan *p = P(h);
     if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step: NULL argument");
     return step_common(p, V, W, ldv, k, lambda, resnorm, converged, S(stream), !lambda && !resnorm && !converged);
+}
+
+int dmrg_davidson_step_given_w(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, double *lambda,
+                               double *resnorm, int32_t *converged, void *stream) {
+    if (!h) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    if (!V || !W || !k) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_given_w: NULL argument");
+    return step_common(p, V, W, ldv, k, lambda, resnorm, converged, S(stream), !lambda && !resnorm && !converged, true);
+}
+
+int dmrg_partition_outputs(int32_t n_outputs, const int64_t *cost, int32_t n_ranks, int32_t *owner) {
+    if (n_outputs < 0 || n_ranks < 1 || !cost || !owner) return fail(nullptr, DMRG_E_INVALID_ARG, "partition_outputs: bad argument");
+    std::vector<long long> c(cost, cost + n_outputs);
+    partition_outputs(n_outputs, c.data(), n_ranks, owner);
+    return DMRG_OK;
+}
+
+int dmrg_get_shard(dmrg_handle_t h, int32_t *owner) {
+    if (!h || !owner) return DMRG_E_INVALID_ARG;
+    Plan *p = P(h);
+    for (size_t q = 0; q < p->owner.size(); q++) owner[q] = p->owner[q];
+    return DMRG_OK;
 }
 
 int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, const double *v_in_host,

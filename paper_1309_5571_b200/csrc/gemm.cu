@@ -551,7 +551,8 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     // bits 0-15 SM id, 16-31 k-tiles of the unit, 32-47 CTA, 48 stage-1 unit, 49 split-K unit, 50 wrote C
                     tr[3] = smid() | ((unsigned long long)u.kt_count << 16) | ((unsigned long long)blockIdx.x << 32) |
                             ((unsigned long long)(u.signal >= 0) << 48) | ((unsigned long long)(u.n_split > 1) << 49) |
-                            ((unsigned long long)writes_c << 50);
+                            ((unsigned long long)writes_c << 50) | ((unsigned long long)((h->ext_m + 7) >> 3) << 52) |
+                            ((unsigned long long)((h->ext_n + 7) >> 3) << 56);      // bits 52-55 / 56-59: sub-tile rows / columns with data
                 }
 #pragma unroll
                 for (int q = 0; q < 8; q++) { acc[q][0] = 0.0; acc[q][1] = 0.0; }

@@ -137,6 +137,7 @@ struct Plan {
     long long n = 0;
     std::vector<int> pairL, pairR;
     std::vector<long long> segOff;
+    std::vector<int> owner;             // output sharding: rank that projects each output segment (all 0 without sharding)
     // device memory
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
     double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
@@ -184,6 +185,7 @@ void set_global_error(const std::string &s);
 int fail(Plan *p, int code, const std::string &msg);
 
 // plan.cu
+void partition_outputs(int n_outputs, const long long *cost, int n_ranks, int *owner);
 int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out);
 void plan_free(Plan *p);
 
@@ -197,7 +199,7 @@ cudaError_t gemm_kernel_setup();
 // davidson.cu
 void dav_setup(Plan *p);
 int dav_init(Plan *p, const double *x0, int argmin_start, double *V, double *W, long long ldv, cudaStream_t st);
-int dav_enqueue_step(Plan *p, double *V, double *W, long long ldv, int k, cudaStream_t st, int *k_next);
+int dav_enqueue_step(Plan *p, double *V, double *W, long long ldv, int k, cudaStream_t st, int *k_next, bool skip_apply = false);
 int dav_ritz(Plan *p, const double *V, long long ldv, int k, double *x_out, cudaStream_t st);
 int dav_gemv_trans(Plan *p, const double *V, long long ldv, int k, const double *w, double *out, cudaStream_t st);
 int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s, double *t, double *nrm2, cudaStream_t st);

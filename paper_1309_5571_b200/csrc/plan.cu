@@ -156,6 +156,22 @@ int check_op(Plan *p, const char *name, const dmrg_block_op &op, const std::vect
 
 }  // namespace
 
+// ---------------------------------------------------------------- output sharding
+// PAPER.md:L342 "all records of the same output on the same [device]", L362 (Alg. 5 step 1: FLOP workload per output):
+// longest-processing-time assignment of the outputs to ranks -- outputs by descending cost (ties: lower index), each to the
+// least loaded rank (ties: lower rank).  Pure host arithmetic: every rank computes the same table.
+void partition_outputs(int n_outputs, const long long *cost, int n_ranks, int *owner) {
+    std::vector<int> ord(n_outputs);
+    for (int q = 0; q < n_outputs; q++) ord[q] = q;
+    std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+    std::vector<long long> load(std::max(n_ranks, 1), 0);
+    for (int q : ord) {
+        int best = 0;
+        for (int r = 1; r < n_ranks; r++) if (load[r] < load[best]) best = r;
+        owner[q] = best; load[best] += cost[q];
+    }
+}
+
 // ---------------------------------------------------------------- plan_build
 #define CUDA_TRY(p, x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) { \
     plan_free(p); return fail(nullptr, (e__ == cudaErrorMemoryAllocation) ? DMRG_E_ALLOC : DMRG_E_CUDA, \
@@ -194,6 +210,9 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     if (p->opt.max_iter <= 0) p->opt.max_iter = 2000;
     if (p->opt.reorth <= 0) p->opt.reorth = 1;
     if (p->opt.check_every <= 0) p->opt.check_every = 8;
+    if (p->opt.shard_count < 0 || (p->opt.shard_count > 1 && (p->opt.shard_rank < 0 || p->opt.shard_rank >= p->opt.shard_count))) {
+        delete p; return fail(nullptr, DMRG_E_INVALID_ARG, "options: need 0 <= shard_rank < shard_count");
+    }
     if (p->opt.max_rhs <= 0) p->opt.max_rhs = 1;
     if (p->opt.max_rhs > BMAX) { delete p; return fail(nullptr, DMRG_E_INVALID_ARG, "options: max_rhs must be 1..4"); }
     p->max_rhs = p->opt.max_rhs;
@@ -372,6 +391,24 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         }
     }
 
+    // ---- output sharding (options.shard_count > 1): this plan projects only the output segments its rank owns
+    const std::vector<Record> all_recs = recs;         // diag(H_SB) needs every record on every rank
+    p->owner.assign(P, 0);
+    if (p->opt.shard_count > 1) {
+        std::vector<long long> cost(P, 0);
+        for (const Record &r : recs) {
+            const long long di = p->dimL[p->pairL[r.in_pair]], dk = p->dimR[p->pairR[r.in_pair]];
+            const long long dj = p->dimL[p->pairL[r.out_pair]], dl = p->dimR[p->pairR[r.out_pair]];
+            if (r.B < 0) cost[r.out_pair] += 2 * dj * di * dk;
+            else if (r.A < 0) cost[r.out_pair] += 2 * di * dk * dl;
+            else cost[r.out_pair] += std::min(2 * di * dk * dl + 2 * dj * di * dl, 2 * dj * di * dk + 2 * dj * dk * dl);
+        }
+        partition_outputs(P, cost.data(), p->opt.shard_count, p->owner.data());
+        std::vector<Record> mine;
+        for (const Record &r : recs) if (p->owner[r.out_pair] == p->opt.shard_rank) mine.push_back(r);
+        recs.swap(mine);
+    }
+
     // ---- stage-1 tasks / stage-2 items; association order by FLOP (A24)
     std::vector<GemmItem> items1, items2;
     std::vector<TaskHost> tasks1, tasks2;
@@ -440,6 +477,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     for (auto &v : out_items)
         std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return (a.dep < 0) > (b.dep < 0); });
     for (int op = 0; op < P; op++) {
+        if (p->opt.shard_count > 1 && p->owner[op] != p->opt.shard_rank) continue;    // not ours: y segment left untouched
         TaskHost t{};
         t.c_base = BASE_Y; t.c_kind = C_ROWMAJOR; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
         t.M = p->dimL[p->pairL[op]]; t.N = p->dimR[p->pairR[op]];
@@ -480,7 +518,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         if (const char *e = getenv("DMRG_TAIL_LO")) lo = atof(e);
         std::vector<long long> vol(P, 0); long long tot2 = 0;
         std::vector<long long> volall(P, 0);
-        for (int op = 0; op < P; op++) { vol[op] = (long long)ktiles(items2, tasks2[op]) * ntiles(tasks2[op]); tot2 += vol[op]; volall[op] = vol[op]; }
+        for (const TaskHost &t : tasks2) { const int op = t.out_pair; vol[op] = (long long)ktiles(items2, t) * ntiles(t); tot2 += vol[op]; volall[op] = vol[op]; }   // (a sharded plan holds only its own outputs)
         for (const TaskHost &t : tasks1) volall[t.out_pair] += (long long)ktiles(items1, t) * ntiles(t);
         std::vector<int> ord(P);
         for (int op = 0; op < P; op++) ord[op] = op;
@@ -607,7 +645,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, cudaGetLastError());
 
     // ---- diag(H_SB) (A14): records with (i,k) == (j,l)
-    for (const Record &r : recs) {
+    for (const Record &r : all_recs) {
         if (r.in_pair != r.out_pair) continue;
         DiagJob dj{};
         dj.seg_off = p->segOff[r.in_pair];
