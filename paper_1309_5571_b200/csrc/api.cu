@@ -176,6 +176,7 @@ int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, 
     if (*k < 1 || *k > p->opt.k_max || ldv < p->n) return fail(p, DMRG_E_INVALID_ARG, "davidson_step_host: k or ldv out of range");
     cudaStream_t st = S(stream);
     // a run that has already converged makes the step a no-op: do not overwrite a column dmrg_ritz_vector still needs
+    if (v_in_host) p->ximg_src = nullptr;       // the newest basis vector comes from the caller: its tile images are not current
     if (v_in_host && p->state_host->done != 1)
         cudaMemcpyAsync(V + (long long)(*k - 1) * ldv, v_in_host, sizeof(double) * p->n, cudaMemcpyHostToDevice, st);
     p->w_out_host = w_out_host;
@@ -222,6 +223,7 @@ int dmrg_set_small(dmrg_handle_t h, const double *B_host, void *stream) {
     int rc = read_state(p, S(stream));
     if (rc != DMRG_OK) return rc;
     const int km = p->opt.k_max;
+    p->ximg_src = nullptr;      // a resumed state: trust nothing cached about the caller's basis
     memset(p->state_host->B, 0, sizeof(p->state_host->B));
     for (int i = 0; i < km; i++) for (int j = 0; j < km; j++) p->state_host->B[i * KMAX + j] = B_host[i * km + j];
     p->state_host->e_k = 0;   // the kept eigenvectors no longer belong to this B

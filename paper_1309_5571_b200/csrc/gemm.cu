@@ -277,7 +277,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
                     const int *__restrict__ done_flag, int yvec, unsigned long long *__restrict__ trace,
                     Prefetch pf, int *__restrict__ err, const XSeg *__restrict__ xsegs, int n_xsegs,
-                    const double *__restrict__ x, long long n, RhsInfo rh) {
+                    const double *__restrict__ x, long long n, RhsInfo rh, int skip_phase0) {
     if (done_flag && *done_flag) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *stage_base = reinterpret_cast<double *>(smem_raw);
@@ -303,7 +303,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     // Phase 0: the caller's vector -> tile images (both operand roles), shared out over all CTAs; a CTA publishes its share
     // (CTRL_XREADY) and the producers wait for all shares before their first copy.  Every CTA of the grid is resident
     // (the grid is one wave), and each writes its share before it waits for anything.
-    {
+    if (!skip_phase0) {        // (skipped when the caller has just written the images itself: scale_img_kernel, davidson.cu)
         const long long share = (n + gridDim.x - 1) / gridDim.x, lo = share * blockIdx.x;
         const XSeg *segs = xsegs;
         if ((size_t)n_xsegs * sizeof(XSeg) <= (size_t)STAGES * STAGE_DOUBLES * 8) {     // the segment table fits the (still idle) ring
@@ -316,16 +316,18 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         for (int r = 0; r < nrhs; r++)
             ximg_share(segs, n_xsegs, x + r * rh.x_ld, lo, min(n, lo + share), bases.p[BASE_XP] + r * rh.stride[BASE_XP],
                        bases.p[BASE_XQ] + r * rh.stride[BASE_XQ], tid);
+        fence_proxy_async();
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) atomicAdd(&ctrl[CTRL_XREADY], 1);
+    } else {
+        __syncthreads();       // the mbarrier initialisation above
     }
-    fence_proxy_async();
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) atomicAdd(&ctrl[CTRL_XREADY], 1);
     if (ctr && tid == 0) ctr[1] = globaltimer();
 
     if (warp == CONSUMERS / 32) {
         // ================================================= producer
-        if (lane == 0) {
+        if (lane == 0 && !skip_phase0) {
             long long spins = 0;
             while (ld_acquire(&ctrl[CTRL_XREADY]) < (int)gridDim.x) {
                 __nanosleep(32);
@@ -580,7 +582,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
 typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int,
-                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo);
+                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo, int);
 struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
     {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},     // default: two CTAs per SM, each able to saturate the DMMA pipes alone
@@ -607,7 +609,10 @@ cudaError_t gemm_kernel_setup() {
 }
 
 int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in,
-            int nrhs, long long ldx, long long ldy) {
+            int nrhs, long long ldx, long long ldy, bool trust_images) {
+    // the tile images of x are current only if the library wrote them itself for exactly this vector (Plan::ximg_src)
+    const int skip_phase0 = (trust_images && nrhs == 1 && p->ximg_src == x) ? 1 : 0;
+    p->ximg_src = nullptr;
     if (nrhs < 1 || nrhs > p->max_rhs) return fail(p, DMRG_E_INVALID_ARG, "apply_H: more right-hand sides than options.max_rhs");
     BasePtrs b;
     b.p[BASE_XP] = p->ximg_p;
@@ -631,7 +636,7 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
         const int grid = (int)std::min<long long>((long long)n_units * nrhs, (long long)g_ctas_per_sm * p->sm_count);   // persistent: one wave
         g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
                                                               p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
-                                                              p->xsegs, p->n_xsegs, x, p->n, rh);
+                                                              p->xsegs, p->n_xsegs, x, p->n, rh, skip_phase0);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

@@ -142,6 +142,10 @@ struct Plan {
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
     double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
     XSeg *xsegs = nullptr; int n_xsegs = 0;
+    // the vector whose tile images are current because the library itself just wrote both (dmrg_davidson_step: line 14 writes
+    // the appended vector and its images); consumed by the next projection of exactly that vector inside a step, cleared by
+    // every other entry point that may see a different or modified vector
+    const double *ximg_src = nullptr;
     int *counters = nullptr;
     GemmItem *items = nullptr;          // stage-1 items, then stage-2 items
     GemmUnit *units = nullptr;          // ticket order: stage-1 units, then stage-2 units
@@ -174,7 +178,7 @@ struct Plan {
     cudaEvent_t ev_apply = nullptr, ev_side = nullptr;
     // CUDA graphs of dmrg_davidson_step, one per (V, W, ldv, basis size)
     typedef std::tuple<const void *, const void *, long long, int> GraphKey;
-    struct GraphEntry { cudaGraphExec_t exec; int k_next; int launches; };
+    struct GraphEntry { cudaGraphExec_t exec; int k_next; int launches; const double *img_src; };
     std::map<GraphKey, GraphEntry> graphs;
     // one call at a time: a hot call on another stream than the previous one first waits for this event
     cudaEvent_t ev_last = nullptr; cudaStream_t last_stream = nullptr; bool last_valid = false;
@@ -207,7 +211,7 @@ int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s
 // into L2 for the kernel that follows (the Davidson basis for line 3), while the launch drains and HBM is idle.
 struct Prefetch { const double *base = nullptr; long long ld = 0, rows = 0; int cols = 0, first_ticket = 0, n_ctas = 0; };
 int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf = nullptr,
-            int nrhs = 1, long long ldx = 0, long long ldy = 0);
+            int nrhs = 1, long long ldx = 0, long long ldy = 0, bool trust_images = false);
 
 // block.cu
 int block_alloc(Plan *p);
