@@ -136,6 +136,25 @@ typedef struct {
                                           this plan since it was created (host-side count) */
 } dmrg_stats;
 
+/* The superblock in the l-1-1-r strategy (Eq. 12-13; Alg. 2):
+ *   H_SB = sum_alpha A_alpha^(l) (x) a_alpha (x) b_alpha (x) B_alpha^(r)
+ * for the spin-1/2 Heisenberg chain, expressed by the operators of the four subsystems: block l, site 1, site 2, block r.
+ * The caller gives the UN-enlarged blocks: H (block-diagonal), Sz and S+ of the block's boundary site (the last site of l,
+ * the first site of r), labels = 2 S_z (any integer unit in which S+ of a site shifts the label by +2; the sites carry
+ * labels -1, +1).  Quadruplets (reading A35): H_l 1 1 1, 1 1 1 H_r, and for each of the three bonds l-site1, site1-site2,
+ * site2-r the terms J/2 (S+ S- + S- S+) + J Delta Sz Sz.  Sector by sector these are Eq. 11 records on the block operators
+ * themselves (largest matrix O(m^2) instead of O((2m)^2)), and the bond between the two sites needs no GEMM.
+ * Flat vector (reading A36): left composite sectors (s, sigma1) at index 2 s + sigma1 (down = 0, up = 1), right composite
+ * sectors (sigma2, s') at index sigma2 * n_r + s'; segments = admissible pairs sorted by (left, right) composite index, each
+ * row-major d_l(s) x d_r(s').  dmrg_get_layout reports the composite indices. */
+typedef struct {
+    double        J, Delta;
+    dmrg_sectors  left, right;             /* sectors of block l and block r (n_labels = 1)            */
+    dmrg_block_op H_l, Sz_l, Sp_l;         /* H_l block-diagonal; Sz_l block-diagonal; S+_l shifts +2  */
+    dmrg_block_op H_r, Sz_r, Sp_r;
+    int32_t       target_twice_sz;
+} dmrg_problem_l11r;
+
 typedef struct dmrg_plan *dmrg_handle_t;
 
 /* ---- plan -------------------------------------------------------------------------- */
@@ -149,6 +168,8 @@ typedef struct dmrg_plan *dmrg_handle_t;
  * synchronises before returning.  opts may be NULL (k_max 20, tol 1e-10, max_iter 2000,
  * reorth 1).  On failure *out = NULL and dmrg_last_error(NULL) has the reason. */
 int dmrg_plan_create(const dmrg_problem *problem, const dmrg_options *opts, dmrg_handle_t *out);
+/* Same, for the l-1-1-r strategy; every other entry point (dmrg_apply_H, the Davidson calls, ...) works on the handle. */
+int dmrg_plan_create_l11r(const dmrg_problem_l11r *problem, const dmrg_options *opts, dmrg_handle_t *out);
 int dmrg_plan_destroy(dmrg_handle_t h);
 
 /* Flat-vector layout.  Any output pointer may be NULL.  left_sector/right_sector/seg_offset

@@ -26,7 +26,7 @@ EXPORTS = [
     "dmrg_probe_fp64_peak", "dmrg_probe_hbm_read", "dmrg_set_timing", "dmrg_get_timing", "dmrg_get_unit_trace", "dmrg_version",
     "dmrg_apply_H_multi", "dmrg_block_init", "dmrg_block_step", "dmrg_block_ritz", "dmrg_block_get_small",
     "dmrg_block_lowest_eigenpairs",
-    "dmrg_partition_outputs", "dmrg_get_shard", "dmrg_davidson_step_given_w",
+    "dmrg_plan_create_l11r", "dmrg_partition_outputs", "dmrg_get_shard", "dmrg_davidson_step_given_w",
     "dmrg_density_matrix", "dmrg_sector_eig", "dmrg_select_states", "dmrg_rotate_op", "dmrg_infinite_heisenberg",
 ]
 
@@ -50,6 +50,12 @@ class _IdmrgOptions(C.Structure):
 class _BlockOp(C.Structure):
     _fields_ = [("n_blocks", C.c_int32), ("src", C.POINTER(C.c_int32)), ("dst", C.POINTER(C.c_int32)),
                 ("offset", C.POINTER(C.c_int64)), ("ld", C.POINTER(C.c_int32)), ("data", C.c_void_p)]
+
+
+class _ProblemL11r(C.Structure):
+    _fields_ = [("J", C.c_double), ("Delta", C.c_double), ("left", _Sectors), ("right", _Sectors),
+                ("H_l", _BlockOp), ("Sz_l", _BlockOp), ("Sp_l", _BlockOp), ("H_r", _BlockOp), ("Sz_r", _BlockOp), ("Sp_r", _BlockOp),
+                ("target_twice_sz", C.c_int32)]
 
 
 _OP_NAMES = ["H_L", "H_R", "Sz_L", "Sp_L", "Sz_R", "Sp_R", "Cup_L", "Cdn_L", "Cup_R", "Cdn_R", "D_L", "D_R"]
@@ -122,6 +128,7 @@ def load_library():
         "dmrg_block_ritz": [vp, vp, vp, i64, i32, i32, vp, i64, vp],
         "dmrg_block_get_small": [vp, i32, pdbl, pdbl, vp],
         "dmrg_block_lowest_eigenpairs": [vp, i32, vp, i64, vp, i64, pdbl, pdbl, pi32, pi32, vp],
+        "dmrg_plan_create_l11r": [C.POINTER(_ProblemL11r), C.POINTER(_Options), C.POINTER(vp)],
         "dmrg_partition_outputs": [i32, pi64, i32, pi32],
         "dmrg_get_shard": [vp, pi32],
         "dmrg_davidson_step_given_w": [vp, vp, vp, i64, pi32, pdbl, pdbl, pi32, vp],
@@ -243,6 +250,30 @@ class Plan:
         opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), int(seed), 0, int(check_every), int(bool(reserve_basis)), int(shard_rank), int(shard_count), int(max_rhs))
         h = C.c_void_p()
         rc = self._lib.dmrg_plan_create(C.byref(pr), C.byref(opt), C.byref(h))
+        self._finish(rc, h, k_max)
+
+    @classmethod
+    def from_l11r(cls, left_block, right_block, J: float, Delta: float, target_twice_sz: int = 0, k_max: int = 20, tol: float = 1e-10,
+                  max_iter: int = 2000, reorth: int = 1, max_rhs: int = 1, device: Optional[str] = None):
+        """Plan of the l-1-1-r strategy (dmrg_plan_create_l11r).  Blocks: objects with .sectors (labels = 2 S_z, dims) and the
+        sector-blocked operators .H, .Sz, .Sp of the UN-enlarged block (dmrg_inputs containers)."""
+        torch = _torch()
+        self = cls.__new__(cls)
+        self._lib = load_library(); self._keep = []
+        self.device = torch.device(device or "cuda:0")
+        torch.cuda.set_device(self.device)
+        pr = _ProblemL11r()
+        pr.J, pr.Delta, pr.target_twice_sz = float(J), float(Delta), int(target_twice_sz)
+        pr.left, pr.right = self._sectors(left_block.sectors), self._sectors(right_block.sectors)
+        pr.H_l, pr.Sz_l, pr.Sp_l = self._block_op(left_block.H), self._block_op(left_block.Sz), self._block_op(left_block.Sp)
+        pr.H_r, pr.Sz_r, pr.Sp_r = self._block_op(right_block.H), self._block_op(right_block.Sz), self._block_op(right_block.Sp)
+        opt = _Options(int(k_max), float(tol), int(max_iter), int(reorth), 1, 0, 8, 0, 0, 0, int(max_rhs))
+        h = C.c_void_p()
+        rc = self._lib.dmrg_plan_create_l11r(C.byref(pr), C.byref(opt), C.byref(h))
+        self._finish(rc, h, k_max)
+        return self
+
+    def _finish(self, rc, h, k_max):
         if rc != DMRG_OK:
             raise DmrgError(rc, (self._lib.dmrg_last_error(None) or b"").decode())
         self._h = h

@@ -49,6 +49,37 @@ int dmrg_plan_create(const dmrg_problem *problem, const dmrg_options *opts, dmrg
     return rc;
 }
 
+int dmrg_plan_create_l11r(const dmrg_problem_l11r *pr, const dmrg_options *opts, dmrg_handle_t *out) {
+    if (!out) return fail(nullptr, DMRG_E_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!pr || pr->left.n_labels != 1 || pr->right.n_labels != 1 || pr->left.n_sectors < 0 || pr->right.n_sectors < 0 ||
+        (pr->left.n_sectors && (!pr->left.labels || !pr->left.dims)) || (pr->right.n_sectors && (!pr->right.labels || !pr->right.dims)))
+        return fail(nullptr, DMRG_E_INVALID_ARG, "l11r problem: NULL or sectors with other than one label");
+    const int nl = pr->left.n_sectors, nr = pr->right.n_sectors;
+    const dmrg_block_op *ops[6] = {&pr->H_l, &pr->Sz_l, &pr->Sp_l, &pr->H_r, &pr->Sz_r, &pr->Sp_r};
+    for (int q = 0; q < 6; q++) {           // block shapes and label shifts (diagonal: 0; S+: +2)
+        const dmrg_block_op &o = *ops[q]; const dmrg_sectors &sec = q < 3 ? pr->left : pr->right;
+        if (o.n_blocks < 0 || (o.n_blocks && (!o.src || !o.dst || !o.offset || !o.ld || !o.data))) return fail(nullptr, DMRG_E_INVALID_ARG, "l11r problem: bad operator arrays");
+        for (int b = 0; b < o.n_blocks; b++) {
+            if (o.src[b] < 0 || o.src[b] >= sec.n_sectors || o.dst[b] < 0 || o.dst[b] >= sec.n_sectors) return fail(nullptr, DMRG_E_SECTOR, "l11r problem: block sector index out of range");
+            if (o.ld[b] < sec.dims[o.src[b]]) return fail(nullptr, DMRG_E_SECTOR, "l11r problem: ld smaller than dims[src]");
+            if (sec.labels[o.dst[b]] - sec.labels[o.src[b]] != ((q % 3 == 2) ? 2 : 0)) return fail(nullptr, DMRG_E_SECTOR, "l11r problem: H, Sz must keep the label, S+ must raise it by 2");
+        }
+    }
+    // composite sectors: left (s, sigma1) at 2 s + sigma1, right (sigma2, s') at sigma2 * n_r + s'   (down = 0 / label -1, up = 1 / +1)
+    std::vector<int32_t> labL(2 * nl), dimL(2 * nl), labR(2 * nr), dimR(2 * nr);
+    for (int s = 0; s < nl; s++) for (int g = 0; g < 2; g++) { labL[2 * s + g] = pr->left.labels[s] + (g ? 1 : -1); dimL[2 * s + g] = pr->left.dims[s]; }
+    for (int g = 0; g < 2; g++) for (int s = 0; s < nr; s++) { labR[g * nr + s] = pr->right.labels[s] + (g ? 1 : -1); dimR[g * nr + s] = pr->right.dims[s]; }
+    dmrg_problem lr; memset(&lr, 0, sizeof(lr));
+    lr.model = DMRG_HEISENBERG; lr.J = pr->J; lr.Delta = pr->Delta;
+    lr.left = {1, 2 * nl, labL.data(), dimL.data()}; lr.right = {1, 2 * nr, labR.data(), dimR.data()};
+    lr.target = &pr->target_twice_sz;
+    Plan *p = nullptr;
+    int rc = plan_build(&lr, opts, &p, pr);
+    *out = reinterpret_cast<dmrg_handle_t>(p);
+    return rc;
+}
+
 int dmrg_plan_destroy(dmrg_handle_t h) {
     if (!h) return DMRG_E_INVALID_ARG;
     cudaDeviceSynchronize();

@@ -181,9 +181,26 @@ __device__ __forceinline__ void disp_nj(int mi, int nj, double (&acc)[8][2], con
 // Epilogue of one warp: its TH x TW accumulator block -> C (row-major caller vector, or the tile images stage 2 loads).
 // sr0 / sc0: first sub-tile row / column of the warp; gq, tg: DMMA fragment coordinates of the lane.
 template <int TH, int TW>
-__device__ __forceinline__ void store_c(const double (&acc)[8][2], const GemmUnit &u, double *C, int sr0, int sc0, int gq, int tg, int yvec) {
+__device__ __forceinline__ void store_c(double (&acc)[8][2], const GemmUnit &u, double *C, int sr0, int sc0, int gq, int tg, int yvec,
+                                        const AxpyItem *__restrict__ axpy, const double *__restrict__ xr) {
     if (u.c_kind == C_ROWMAJOR) {
         const bool cvec = u.c_vec2 && (u.c_base != BASE_Y || yvec);
+        // l-1-1-r: scaled copies of input segments of the same shape (the bond between the two sites)
+        for (int q = 0; q < u.axpy_count; q++) {
+            const AxpyItem it = axpy[u.axpy_begin + q];
+            const double *xs = xr + it.x_off;
+#pragma unroll
+            for (int i = 0; i < TH; i++) {
+                const int row = u.m0 + (sr0 + i) * 8 + gq;
+                if (row >= u.M) continue;
+#pragma unroll
+                for (int j = 0; j < TW; j++) {
+                    const int col = u.n0 + (sc0 + j) * 8 + 2 * tg;
+                    if (col < u.N) acc[i * TW + j][0] = fma(it.c, xs[(long long)row * u.ldc + col], acc[i * TW + j][0]);
+                    if (col + 1 < u.N) acc[i * TW + j][1] = fma(it.c, xs[(long long)row * u.ldc + col + 1], acc[i * TW + j][1]);
+                }
+            }
+        }
 #pragma unroll
         for (int i = 0; i < TH; i++) {
             const int row = u.m0 + (sr0 + i) * 8 + gq;
@@ -277,7 +294,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
                     const int *__restrict__ done_flag, int yvec, unsigned long long *__restrict__ trace,
                     Prefetch pf, int *__restrict__ err, const XSeg *__restrict__ xsegs, int n_xsegs,
-                    const double *__restrict__ x, long long n, RhsInfo rh, int skip_phase0) {
+                    const double *__restrict__ x, long long n, RhsInfo rh, int skip_phase0, const AxpyItem *__restrict__ axpy) {
     if (done_flag && *done_flag) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *stage_base = reinterpret_cast<double *>(smem_raw);
@@ -540,10 +557,11 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     pending = counters + h->rhs * rh.n_counters + u.tile_id; pending_g = g;
                 } else {
                     double *C = s_base[u.c_base] + h->rhs * s_stride[u.c_base] + u.c_off;
-                    if (layout == 0) store_c<4, 2>(acc, u, C, sr0, sc0, gq, tg, yvec);
-                    else if (layout == 1) store_c<2, 4>(acc, u, C, sr0, sc0, gq, tg, yvec);
-                    else if (layout == 2) store_c<8, 1>(acc, u, C, sr0, sc0, gq, tg, yvec);
-                    else store_c<1, 8>(acc, u, C, sr0, sc0, gq, tg, yvec);
+                    const double *xr = x + h->rhs * rh.x_ld;
+                    if (layout == 0) store_c<4, 2>(acc, u, C, sr0, sc0, gq, tg, yvec, axpy, xr);
+                    else if (layout == 1) store_c<2, 4>(acc, u, C, sr0, sc0, gq, tg, yvec, axpy, xr);
+                    else if (layout == 2) store_c<8, 1>(acc, u, C, sr0, sc0, gq, tg, yvec, axpy, xr);
+                    else store_c<1, 8>(acc, u, C, sr0, sc0, gq, tg, yvec, axpy, xr);
                     // this tile of a T block is complete: to be published (release: this warp's stores, then its count)
                     if (u.signal >= 0) { pending = ctrl + CTRL_DEP0 + h->rhs * n_deps + u.signal; pending_g = g; }
                 }
@@ -582,7 +600,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
 typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int,
-                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo, int);
+                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo, int, const AxpyItem *);
 struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
     {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},     // default: two CTAs per SM, each able to saturate the DMMA pipes alone
@@ -636,7 +654,7 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
         const int grid = (int)std::min<long long>((long long)n_units * nrhs, (long long)g_ctas_per_sm * p->sm_count);   // persistent: one wave
         g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
                                                               p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
-                                                              p->xsegs, p->n_xsegs, x, p->n, rh, skip_phase0);
+                                                              p->xsegs, p->n_xsegs, x, p->n, rh, skip_phase0, p->axpy);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

@@ -54,7 +54,12 @@ struct GemmUnit {
     int signal;               // T-block ready counter to bump once this tile of T is written (-1: none)
     int cost;                 // scheduling weight (DMMA count + per-k-tile overhead)
     int item0, k00;           // where kt_begin falls: item index inside the unit's item list and k offset inside that item
+    int axpy_begin, axpy_count;   // l-1-1-r: scaled copies of input segments added to this output (C_ROWMAJOR units only)
 };
+
+// l-1-1-r strategy: the bond between the two single sites maps a segment onto a segment of the same
+// shape with a scalar -- no GEMM: y_seg += c * x[x_off ...] in the epilogue of the output tile.
+struct AxpyItem { long long x_off; double c; };
 
 // control words of one apply (device ints): ticket dispenser, finished count, X-image count, then one ready counter per T block
 enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_XREADY = 2, CTRL_DEP0 = 3 };   // XREADY: CTAs whose share of the X images is written
@@ -142,6 +147,7 @@ struct Plan {
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
     double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
     XSeg *xsegs = nullptr; int n_xsegs = 0;
+    AxpyItem *axpy = nullptr;
     // the vector whose tile images are current because the library itself just wrote both (dmrg_davidson_step: line 14 writes
     // the appended vector and its images); consumed by the next projection of exactly that vector inside a step, cleared by
     // every other entry point that may see a different or modified vector
@@ -190,7 +196,7 @@ int fail(Plan *p, int code, const std::string &msg);
 
 // plan.cu
 void partition_outputs(int n_outputs, const long long *cost, int n_ranks, int *owner);
-int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out);
+int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, const dmrg_problem_l11r *l11 = nullptr);
 void plan_free(Plan *p);
 
 // plan.cu: ordering of hot calls of one plan across streams (include/dmrg_b200.h "A plan serves ONE call at a time")

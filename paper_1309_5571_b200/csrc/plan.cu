@@ -91,7 +91,7 @@ struct PoolEntry { long long off; int rows, cols; bool q_role; };
 struct FactorBlk { int src, dst, entry; };          // entry = pool index
 struct Term { bool A_id, B_id; std::vector<FactorBlk> A, B; };
 struct Record { int A, B, in_pair, out_pair; };      // pool entries or -1 (identity)
-struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; int out_pair; uint8_t c_kind; };
+struct TaskHost { uint8_t c_base; long long c_off; int ldc, M, N; int item_begin, item_count; int out_pair; uint8_t c_kind; int axpy_begin = 0, axpy_count = 0; };
 
 
 struct Builder {
@@ -185,7 +185,7 @@ static cudaError_t dev_alloc(Plan *p, T **ptr, long long count) {
     return e;
 }
 
-int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
+int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, const dmrg_problem_l11r *l11) {
     *out = nullptr;
     if (!pr) return fail(nullptr, DMRG_E_INVALID_ARG, "problem is NULL");
     if (pr->model != DMRG_HEISENBERG && pr->model != DMRG_HUBBARD)
@@ -364,6 +364,64 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         }
     }
 
+    // ---- l-1-1-r strategy (Eq. 12-13): the sectors given to this function are the COMPOSITE ones -- left
+    // (s, sigma1) at index 2 s + sigma1, right (sigma2, s') at index sigma2 * n_r + s' (down = 0, up = 1) -- and the operator
+    // quadruplets A (x) a (x) b (x) B of the Heisenberg chain reduce, sector by sector, to Eq. 11 records on the UN-enlarged
+    // block operators: the 2 x 2 site operators have one non-zero element per row, so a (x) b only selects the segment and
+    // scales it.  H_l 1 1 1 + bond(l, site 1) is a left-only term with blocks between composite sectors of equal label,
+    // 1 1 1 H_r + bond(site 2, r) a right-only term, and the bond between the two sites needs no GEMM at all: scaled copies
+    // of input segments into output segments (axpy items, added in the epilogue of the output tile).
+    std::vector<std::vector<AxpyItem>> out_axpy;
+    if (l11) {
+        const int nl_ = l11->left.n_sectors, nr_ = l11->right.n_sectors;
+        std::vector<int> dl(l11->left.dims, l11->left.dims + nl_), dr(l11->right.dims, l11->right.dims + nr_);
+        const double half = 0.5 * l11->J, zz = l11->J * l11->Delta;
+        auto diag_block = [](const dmrg_block_op &op, int s) { for (int b = 0; b < op.n_blocks; b++) if (op.src[b] == s && op.dst[b] == s) return b; return -1; };
+        Term tl; tl.A_id = false; tl.B_id = true;
+        Term tr; tr.A_id = true; tr.B_id = false;
+        for (int side = 0; side < 2; side++) {
+            const dmrg_block_op &H = side == 0 ? l11->H_l : l11->H_r, &Sz = side == 0 ? l11->Sz_l : l11->Sz_r, &Sp = side == 0 ? l11->Sp_l : l11->Sp_r;
+            const std::vector<int> &dims = side == 0 ? dl : dr;
+            const int ns = (int)dims.size();
+            auto comp = [&](int s, int sg) { return side == 0 ? 2 * s + sg : sg * ns + s; };
+            const bool q = side == 1;          // right factors are Q operands, stored as B^T
+            Term &t = side == 0 ? tl : tr;
+            std::vector<FactorBlk> &list = side == 0 ? t.A : t.B;
+            for (int s = 0; s < ns; s++) {
+                if (dims[s] == 0) continue;
+                const int hb = diag_block(H, s), zb = diag_block(Sz, s);
+                for (int sg = 0; sg < 2; sg++) {     // H_b + J Delta sigma Sz_b on (s, sigma)
+                    const double c = zz * (sg - 0.5);
+                    int e = -1;
+                    if (hb >= 0 && zb >= 0 && c != 0.0) e = bl.add_entry(q, H, hb, dims, q, 1.0, &Sz, zb, c);
+                    else if (hb >= 0) e = bl.add_entry(q, H, hb, dims, q, 1.0);
+                    else if (zb >= 0 && c != 0.0) e = bl.add_entry(q, Sz, zb, dims, q, c);
+                    if (e >= 0) list.push_back({comp(s, sg), comp(s, sg), e});
+                }
+            }
+            if (half != 0.0)
+                for (int b = 0; b < Sp.n_blocks; b++) {   // S+_b S-_site: (s, up) -> (s', down), and the transpose back
+                    const int s0 = Sp.src[b], s1 = Sp.dst[b];
+                    if (!dims[s0] || !dims[s1]) continue;
+                    list.push_back({comp(s0, 1), comp(s1, 0), bl.add_entry(q, Sp, b, dims, q, half)});
+                    list.push_back({comp(s1, 0), comp(s0, 1), bl.add_entry(q, Sp, b, dims, !q, half)});
+                }
+        }
+        terms.push_back(std::move(tl));
+        terms.push_back(std::move(tr));
+        // bond site 1 - site 2: X'(s,s1';s2',s') += c X(s,s1;s2,s')
+        out_axpy.assign(P, {});
+        for (int op = 0; op < P; op++) {
+            const int cl = p->pairL[op], cr = p->pairR[op];
+            const int s = cl / 2, s1 = cl % 2, s2 = cr / nr_, sp = cr % nr_;
+            if (zz != 0.0) out_axpy[op].push_back({p->segOff[op], zz * (s1 - 0.5) * (s2 - 0.5)});
+            if (half != 0.0 && s1 != s2) {           // (up, down) <-> (down, up)
+                auto it = pair_index.find({2 * s + s2, s1 * nr_ + sp});
+                if (it != pair_index.end()) out_axpy[op].push_back({p->segOff[it->second], half});
+            }
+        }
+    }
+
     // ---- operation records, in term order, grouped later by output
     std::vector<Record> recs;
     for (const Term &t : terms) {
@@ -476,12 +534,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     // starting at k = 0 has work before its first T block is complete (order fixed at plan time: deterministic)
     for (auto &v : out_items)
         std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return (a.dep < 0) > (b.dep < 0); });
+    std::vector<AxpyItem> axpy;
     for (int op = 0; op < P; op++) {
         if (p->opt.shard_count > 1 && p->owner[op] != p->opt.shard_rank) continue;    // not ours: y segment left untouched
         TaskHost t{};
         t.c_base = BASE_Y; t.c_kind = C_ROWMAJOR; t.c_off = p->segOff[op]; t.ldc = p->dimR[p->pairR[op]];
         t.M = p->dimL[p->pairL[op]]; t.N = p->dimR[p->pairR[op]];
         t.item_begin = (int)items2.size(); t.item_count = (int)out_items[op].size(); t.out_pair = op;
+        if (!out_axpy.empty()) { t.axpy_begin = (int)axpy.size(); t.axpy_count = (int)out_axpy[op].size(); for (const AxpyItem &a : out_axpy[op]) axpy.push_back(a); }
         for (const GemmItem &it : out_items[op]) items2.push_back(it);
         tasks2.push_back(t);   // outputs without any record are still zero-filled by the kernel
     }
@@ -553,6 +613,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
                     u.c_base = t.c_base; u.c_kind = t.c_kind; u.c_vec2 = vec2(t.c_off, t.ldc);
                     u.signal = signals ? (int)ti : -1;
                     u.cost = u.kt_count * (4 * sub + 64);
+                    u.axpy_begin = t.axpy_begin; u.axpy_count = t.axpy_count;
                     {   // resolve kt_begin to (item, k offset) here, so that the kernel does not walk the item list
                         int skip = u.kt_begin, q = 0;
                         for (; q < t.item_count; q++) {
@@ -620,6 +681,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
     CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->axpy, (long long)axpy.size()));
+    if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
     CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + (long long)p->n_deps * R));
     CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
     if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
@@ -656,6 +719,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
         long long tot = (long long)dj.rows * dj.cols;
         diag_kernel<<<(unsigned)((tot + 255) / 256), 256>>>(dj, p->D);
     }
+    for (int op = 0; op < P && !out_axpy.empty(); op++)          // l-1-1-r: the diagonal part of the site-site bond
+        for (const AxpyItem &a : out_axpy[op]) {
+            if (a.x_off != p->segOff[op]) continue;
+            DiagJob dj{};
+            dj.seg_off = p->segOff[op]; dj.rows = p->dimL[p->pairL[op]]; dj.cols = p->dimR[p->pairR[op]]; dj.c = a.c;
+            const long long tot = (long long)dj.rows * dj.cols;
+            diag_kernel<<<(unsigned)((tot + 255) / 256), 256>>>(dj, p->D);
+        }
     CUDA_TRY(p, cudaGetLastError());
 
     // ---- Davidson scratch
@@ -704,7 +775,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out) {
 void plan_free(Plan *p) {
     if (!p) return;
     cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
-    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs);
+    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs); cudaFree(p->axpy);
     cudaFree(p->items); cudaFree(p->units); cudaFree(p->ctrl); cudaFree(p->trace);
     cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
