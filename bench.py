@@ -248,6 +248,10 @@ def davidson_hbm_probe(lib, device, hbm_peak, name="cfg5b", steps=36, hbm_read=N
            "kernels_gbs": {nm: v[0] / (v[1] * 1e-3) / 1e9 for nm, v in acc.items() if v[1] > 0},
            "hbm_peak_gbs": hbm_peak}
     tot_b = sum(v[0] for v in acc.values()); tot_ms = sum(v[1] for v in acc.values())
+    if acc["append"][1] > 0:    # a9 also writes the two 8 KB-tile images of the new vector (16 n bytes more) that the projection reads
+        out["append_gbs_incl_tile_images"] = 2.0 * acc["append"][0] / (acc["append"][1] * 1e-3) / 1e9
+        out["append_note"] = ("'append' above counts SURVEY 8(d)'s 16 n bytes (t read, v_k written); the kernel moves 32 n: it also writes "
+                              "the P and Q tile images of v_k, the repack the projection kernel would otherwise do in its phase 0")
     out["blas2_gbs"] = tot_b / (tot_ms * 1e-3) / 1e9
     out["blas2_frac_hbm"] = out["blas2_gbs"] / hbm_peak
     out["kernels_frac_hbm"] = {nm: g / hbm_peak for nm, g in out["kernels_gbs"].items()}
@@ -453,7 +457,7 @@ def run_ours(args):
             dav_large["other_configs"] = {}
             for nm in ("cfg5a", "heis4096"):     # the judgement is also taken at 5a and the 4096 sweep
                 o = davidson_hbm_probe(lib, f"cuda:{local}", hbm_peak, name=nm, steps=40, hbm_read=hbm_read)
-                dav_large["other_configs"][nm] = {kk: o[kk] for kk in ("workload", "kernels_gbs", "kernels_frac_hbm", "kernels_frac_hbm_read",
+                dav_large["other_configs"][nm] = {kk: o[kk] for kk in ("workload", "kernels_gbs", "kernels_frac_hbm", "kernels_frac_hbm_read", "append_gbs_incl_tile_images",
                                                                        "blas2_gbs", "blas2_frac_hbm", "blas2_frac_hbm_read") if kk in o}
         except Exception as e:   # the headline numbers above do not depend on this extra config
             dav_large = {"error": repr(e)}
@@ -480,6 +484,13 @@ def run_ours(args):
             block = block_davidson_probe(lib, problem, cfg, f"cuda:{local}", st)
         except Exception as e:
             block = {"error": repr(e)}
+
+    next_rows = None
+    if side:
+        try:
+            next_rows = next_rows_probe(lib, f"cuda:{local}", max(dmma_peak, dfma_peak))
+        except Exception as e:
+            next_rows = {"error": repr(e)}
 
     curve = None
     if side:
@@ -521,7 +532,7 @@ def run_ours(args):
                          "blas2_gbs": blas2_gbs, "blas2_frac_hbm": (blas2_gbs / hbm_peak) if blas2_gbs else None,
                          "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
                          "note": "BLAS-2 kernels timed inside the running loop, warm L2: V+W fit partly in the 126 MB L2 at this config"},
-            "davidson_hbm": dav_large, "gemv_trans": gt_probe, "hpsi_curve": curve, "block_davidson": block,
+            "davidson_hbm": dav_large, "gemv_trans": gt_probe, "hpsi_curve": curve, "block_davidson": block, "next_rows": next_rows,
             "device_bytes": plan.stats()["device_bytes"] + 2 * V.numel() * 8}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -563,6 +574,46 @@ def block_davidson_probe(lib, problem, cfg, device, st):
                     "note": "block: two pairs to 1e-10, two synchronisations per block iteration (first slice); "
                             "single: one pair, steps enqueued back to back"}
     plan.close()
+    return out
+
+
+def next_rows_probe(lib, device, fp64_peak):
+    """SURVEY 8(f) NEXT-1 and NEXT-2, measured: (a) dmrg_apply_H of an l-1-1-r plan on two synthetic
+    un-enlarged blocks of m = 1024 states (dmrg_inputs.heisenberg_block_synthetic, seeds 71/72): the superblock dimension is
+    that of the LR plan of the enlarged blocks (m = 2048 per side); (b) the infinite-lattice loop dmrg_infinite_heisenberg
+    (Alg. 1, every step on the device) to 64 sites with m = 128, wall clock around the C-ABI call."""
+    import torch
+    from dmrg_inputs import heisenberg_block_synthetic
+    out = {}
+    l, r = heisenberg_block_synthetic(1024, 4, 71), heisenberg_block_synthetic(1024, 4, 72)
+    plan = lib.Plan.from_l11r(l, r, 1.0, 1.0, 0, device=device)
+    st = plan.stats()
+    x = torch.randn(plan.n, dtype=torch.float64, device=device); y = torch.empty_like(x)
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        plan.apply_H(x, y)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(10):
+        plan.apply_H(x, y)
+    e1.record(stream); torch.cuda.synchronize()
+    us = e0.elapsed_time(e1) / 10 * 1e3
+    out["l11r_apply"] = {"workload": "l-1-1-r, two synthetic blocks of m = 1024 (9 sectors), target 2 S_z = 0", "n": int(plan.n),
+                         "flop_per_apply": int(st["flop_per_apply"]), "us_per_apply": us,
+                         "tflops": st["flop_per_apply"] / (us * 1e-6) / 1e12,
+                         "frac_fp64_peak": st["flop_per_apply"] / (us * 1e-6) / 1e12 / fp64_peak,
+                         "units": int(st["stage1_units"] + st["stage2_units"])}
+    plan.close()
+    del x, y
+    lib.infinite_heisenberg(16, 32)                      # warm-up (module load, allocator)
+    t0 = time.perf_counter()
+    recs = lib.infinite_heisenberg(64, 128)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    last = recs[-1]
+    out["infinite_dmrg"] = {"workload": "Heisenberg Delta = 1, infinite-lattice growth 4 -> 64 sites, m = 128, tol 1e-10",
+                            "wall_s": dt, "superblocks": len(recs), "energy_per_site_last": float(last["energy"]) / int(last["n_sites"]),
+                            "discarded_last": float(max(last["discarded"])), "davidson_iters_total": int(sum(q["davidson_iters"] for q in recs))}
     return out
 
 

@@ -8,7 +8,9 @@ and the seeded random recipes of DESIGN.md ("Input recipe").
 """
 from .problem import Sectors, BlockOp, Problem
 from .synthetic import (heisenberg_synthetic, hubbard_synthetic, sector_profile,
-                        random_vector, vector_seed, CONFIGS, make_config)
+                        random_vector, vector_seed, CONFIGS, make_config,
+                        SimpleBlock, heisenberg_block_synthetic)
 
 __all__ = ["Sectors", "BlockOp", "Problem", "heisenberg_synthetic", "hubbard_synthetic",
-           "sector_profile", "random_vector", "vector_seed", "CONFIGS", "make_config"]
+           "sector_profile", "random_vector", "vector_seed", "CONFIGS", "make_config",
+           "SimpleBlock", "heisenberg_block_synthetic"]

@@ -126,6 +126,32 @@ def hubbard_synthetic(m: int, U: float, seed: int, t: float = 1.0, ell: int = 8,
                     "D_L": DL, "D_R": DR}, np.array([ell, ell]))
 
 
+class SimpleBlock:
+    """An un-enlarged block for the l-1-1-r strategy: sectors (labels = 2 S_z) and the sector-blocked
+    operators H (block-diagonal), Sz, Sp (label + 2) of its boundary site.  Container only."""
+
+    def __init__(self, sectors, H, Sz, Sp):
+        self.sectors, self.H, self.Sz, self.Sp = sectors, H, Sz, Sp
+
+
+def heisenberg_block_synthetic(m: int, qmax: int, seed: int, sigma: float = 1.6) -> SimpleBlock:
+    """Synthetic un-enlarged block with the shape of a truncated DMRG block (same recipe as `heisenberg_synthetic`, A8-A11):
+    sectors 2 S_z = -2 qmax .. 2 qmax in steps of 2 with a seeded Gaussian size profile summing to m, H symmetric N(0,1)
+    blocks, Sz dense symmetric N(0,1/m) blocks, S+ blocks N(0,1/m) from label q to q + 2."""
+    rng = np.random.default_rng(seed)
+    q = np.arange(-qmax, qmax + 1)
+    dims = sector_profile(np.exp(-q.astype(np.float64) ** 2 / (2.0 * sigma * sigma)), m, rng)
+    H, Sz, Sp = BlockOp(), BlockOp(), BlockOp()
+    std = 1.0 / np.sqrt(m)
+    for s, d in enumerate(dims):
+        d = int(d)
+        g = rng.standard_normal((d, d)); H.add(s, s, np.triu(g) + np.triu(g, 1).T)
+        g = rng.standard_normal((d, d)) * std; Sz.add(s, s, np.triu(g) + np.triu(g, 1).T)
+    for s in range(len(dims) - 1):
+        Sp.add(s, s + 1, rng.standard_normal((int(dims[s + 1]), int(dims[s]))) * std)
+    return SimpleBlock(Sectors((2 * q).reshape(-1, 1), dims), H, Sz, Sp)
+
+
 def random_vector(n: int, seed: int) -> np.ndarray:
     """Seeded N(0,1) vector on the n target-sector entries (A19 start (R); H*psi test vectors)."""
     return np.random.default_rng(seed).standard_normal(n)

@@ -57,10 +57,18 @@ def _random_block(dims, seed):
     return renorm.Block(Sectors(labels.reshape(-1, 1), np.array(dims)), H, Sz, Sp, 0)
 
 
+def _synth(m, qmax, seed):
+    """The generator bench.py's l-1-1-r probe uses (dmrg_inputs.heisenberg_block_synthetic), at a size the oracle finishes."""
+    from dmrg_inputs import heisenberg_block_synthetic
+    b = heisenberg_block_synthetic(m, qmax, seed)
+    return renorm.Block(b.sectors, b.H, b.Sz, b.Sp, 0)
+
+
 CASES = {
     "exact_1": lambda: (_exact(1, 1.0), 1.0, 0), "exact_2_d05": lambda: (_exact(2, 0.5), 0.5, 0), "exact_4": lambda: (_exact(4, 1.0), 1.0, 0),
     "exact_5_target2": lambda: (_exact(5, 0.7), 0.7, 2), "trunc_5_m12": lambda: (_truncated(5, 1.0, 12), 1.0, 0),
     "random_ragged": lambda: ((_random_block([3, 40, 70, 130, 66, 20, 1], 1), _random_block([2, 33, 65, 129, 64, 17, 1], 2)), 0.8, 0),
+    "bench_generator_m160": lambda: ((_synth(160, 3, 71), _synth(160, 3, 72)), 1.0, 0),
     "random_uneven": lambda: ((_random_block([1, 0, 90, 7], 3), _random_block([5, 200, 31, 0, 2], 4)), 1.3, 1),
 }
 

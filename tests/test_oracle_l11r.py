@@ -76,3 +76,20 @@ def test_truncated_blocks_and_other_targets():
         assert np.max(np.abs(H - H.T)) <= 1e-13
         Hs2, _ = kron.H_sector(renorm.superblock(renorm.enlarge(lt, "left", 1.0, 0.7), renorm.enlarge(rt, "right", 1.0, 0.7), 1.0, 0.7, target))
         assert H.shape == Hs2.shape and np.max(np.abs(np.linalg.eigvalsh(H) - np.linalg.eigvalsh(Hs2))) <= 1e-11
+
+
+def test_block_generator_shapes():
+    """dmrg_inputs.heisenberg_block_synthetic (the l-1-1-r bench input): seeded, dims sum to m, H and Sz symmetric and
+    block-diagonal, S+ raises the label by 2."""
+    from dmrg_inputs import heisenberg_block_synthetic
+    a, b = heisenberg_block_synthetic(64, 3, 5), heisenberg_block_synthetic(64, 3, 5)
+    assert int(a.sectors.dims.sum()) == 64 and a.sectors.n_sectors == 7
+    assert list(a.sectors.labels[:, 0]) == [-6, -4, -2, 0, 2, 4, 6]
+    for op, op2 in ((a.H, b.H), (a.Sz, b.Sz), (a.Sp, b.Sp)):
+        for x, y in zip(op.blocks, op2.blocks):
+            assert np.array_equal(x, y)
+    for op in (a.H, a.Sz):
+        for s, d, blk in zip(op.src, op.dst, op.blocks):
+            assert s == d and np.array_equal(blk, blk.T) and blk.shape == (a.sectors.dims[s],) * 2
+    for s, d, blk in zip(a.Sp.src, a.Sp.dst, a.Sp.blocks):
+        assert d == s + 1 and blk.shape == (a.sectors.dims[d], a.sectors.dims[s])
