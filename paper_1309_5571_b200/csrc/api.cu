@@ -199,6 +199,13 @@ int dmrg_get_shard(dmrg_handle_t h, int32_t *owner) {
     return DMRG_OK;
 }
 
+// Device-accessible alias of a pinned host pointer (cudaHostAlloc / cudaHostRegister memory); NULL for pageable memory.
+static void *device_view(const void *host) {
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return (a.type == cudaMemoryTypeHost) ? a.devicePointer : nullptr;
+}
+
 int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, int32_t *k, const double *v_in_host,
                             double *w_out_host, double *lambda, double *resnorm, int32_t *converged, void *stream) {
     if (!h) return DMRG_E_INVALID_ARG;
@@ -208,11 +215,21 @@ int dmrg_davidson_step_host(dmrg_handle_t h, double *V, double *W, int64_t ldv, 
     cudaStream_t st = S(stream);
     // a run that has already converged makes the step a no-op: do not overwrite a column dmrg_ritz_vector still needs
     if (v_in_host) p->ximg_src = nullptr;       // the newest basis vector comes from the caller: its tile images are not current
-    if (v_in_host && p->state_host->done != 1)
-        cudaMemcpyAsync(V + (long long)(*k - 1) * ldv, v_in_host, sizeof(double) * p->n, cudaMemcpyHostToDevice, st);
+    // A pinned (device-accessible) v_in is not copied by the copy engine: loader CTAs of the projection kernel pull it over PCIe
+    // share by share while the other CTAs already work on the segments that have arrived (DMRG_HOST_STREAM=0: staged copy).
+    // Pageable memory, or a plan with axpy terms (l-1-1-r), takes the staged copy.  (Mirroring H v to the host from the
+    // kernel's epilogue was measured too: the scattered 16-byte PCIe writes doubled the step time; w_out stays a D2H copy
+    // on the side stream, under lines 3-13.)
+    static const int host_stream = []() { const char *e = getenv("DMRG_HOST_STREAM"); return e ? atoi(e) : 1; }();
+    const double *v_dev = nullptr;
+    if (v_in_host && host_stream && !p->axpy_count) v_dev = static_cast<const double *>(device_view(v_in_host));
+    if (v_in_host && p->state_host->done != 1) {
+        if (v_dev) p->x_stream = v_dev;
+        else cudaMemcpyAsync(V + (long long)(*k - 1) * ldv, v_in_host, sizeof(double) * p->n, cudaMemcpyHostToDevice, st);
+    }
     p->w_out_host = w_out_host;
     int rc = step_common(p, V, W, ldv, k, lambda, resnorm, converged, st, false);
-    p->w_out_host = nullptr;
+    p->w_out_host = nullptr; p->x_stream = nullptr;
     if (w_out_host) {
         cudaError_t e = cudaStreamSynchronize(p->side);
         if (rc == DMRG_OK && e != cudaSuccess) return fail(p, DMRG_E_CUDA, cudaGetErrorString(e));

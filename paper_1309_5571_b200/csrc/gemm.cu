@@ -115,9 +115,10 @@ struct Producer {
 };
 
 __device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, const long long *stride,
-                                           int rhs, int n_deps, int m0, int n0, int k0, int lane, const int *ctrl, int *err) {
-    const int dep = it->dep;
-    if (dep >= 0) {            // operand is a T block of this launch: wait until all its tiles are written
+                                           int rhs, int n_deps, int m0, int n0, int k0, int lane, const int *ctrl, int *err,
+                                           int xmode) {
+    const int dep = (it->xdep && xmode != 2) ? -1 : it->dep;     // X segments: ready before the first unit unless x is streamed in
+    if (dep >= 0) {            // operand is a T block of this launch (or a streamed X segment): wait until it is all written
         if (lane == 0) {
             const int need = it->dep_need;
             const int *c = ctrl + CTRL_DEP0 + rhs * n_deps + dep;
@@ -294,7 +295,9 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                     int *__restrict__ counters, int *__restrict__ ctrl, int n_units, int n_deps,
                     const int *__restrict__ done_flag, int yvec, unsigned long long *__restrict__ trace,
                     Prefetch pf, int *__restrict__ err, const XSeg *__restrict__ xsegs, int n_xsegs,
-                    const double *__restrict__ x, long long n, RhsInfo rh, int skip_phase0, const AxpyItem *__restrict__ axpy) {
+                    const double *__restrict__ x, long long n, RhsInfo rh, int xmode, const AxpyItem *__restrict__ axpy,
+                    XStream xs) {
+    const int skip_phase0 = xmode != 0;      // xmode 0: phase 0 by all CTAs; 1: images are current; 2: streamed by loader CTAs
     if (done_flag && *done_flag) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *stage_base = reinterpret_cast<double *>(smem_raw);
@@ -339,6 +342,40 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         if (tid == 0) atomicAdd(&ctrl[CTRL_XREADY], 1);
     } else {
         __syncthreads();       // the mbarrier initialisation above
+    }
+    if (xmode == 2 && (int)blockIdx.x < xs.n_loaders) {
+        // Streamed input: x lives in pinned host memory.  A few loader CTAs (few, so that the shares arrive over PCIe in the order
+        // they were requested) pull it share by share in the order of first use, write the tile images and the device copy,
+        // and publish the elements written per segment; the units' X items wait on those counters (begin_item).  A loader
+        // waits for nothing, and joins the others on the units once the share list is empty.
+        __shared__ int s_share;
+        for (;;) {
+            __syncthreads();
+            if (tid == 0) s_share = atomicAdd(&ctrl[CTRL_XSHARE], 1);
+            __syncthreads();
+            const int sh = s_share;
+            if (sh >= xs.n_shares) break;
+            const XShare S = xs.shares[sh];
+            const XSeg sg = xsegs[S.seg];
+            const int KTp = (sg.dk + BK - 1) / BK, KTq = (sg.di + BK - 1) / BK;
+            constexpr int U = 12;
+            double v[U];
+#pragma unroll
+            for (int q = 0; q < U; q++) { const int e = S.lo + tid + q * THREADS; v[q] = e < S.hi ? x[sg.seg_off + e] : 0.0; }
+#pragma unroll
+            for (int q = 0; q < U; q++) {
+                const int e = S.lo + tid + q * THREADS;
+                if (e >= S.hi) break;
+                const int r = e / sg.dk, c = e - r * sg.dk;
+                bases.p[BASE_XP][sg.xp_off + ((long long)(r / BM) * KTp + c / BK) * IMG + img_p_index(r % BM, c % BK)] = v[q];
+                bases.p[BASE_XQ][sg.xq_off + ((long long)(c / BN) * KTq + r / BK) * IMG + img_q_index(r % BK, c % BN)] = v[q];
+                if (xs.x_copy) xs.x_copy[sg.seg_off + e] = v[q];
+            }
+            fence_proxy_async();
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) atomicAdd(&ctrl[CTRL_DEP0 + S.seg], S.hi - S.lo);
+        }
     }
     if (ctr && tid == 0) ctr[1] = globaltimer();
 
@@ -400,7 +437,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 continue;
             }
             Producer pr{};
-            begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, k00, lane, ctrl, err);
+            begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, k00, lane, ctrl, err, xmode);
             for (int t = 0; t < KT; t++) {
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
@@ -418,7 +455,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 g++;
                 if (pr.k0 >= pr.K && t + 1 < KT) {
                     p_item++;
-                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, 0, lane, ctrl, err);
+                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, 0, lane, ctrl, err, xmode);
                 }
             }
             if (reducer) {
@@ -600,7 +637,8 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
 
 // kernel variants (selected once per process; DMRG_GEMM_VARIANT overrides the default for experiments)
 typedef void (*gemm_fn)(const GemmUnit *, const GemmItem *, BasePtrs, int *, int *, int, int, const int *, int,
-                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo, int, const AxpyItem *);
+                        unsigned long long *, Prefetch, int *, const XSeg *, int, const double *, long long, RhsInfo, int, const AxpyItem *,
+                        XStream);
 struct Variant { const char *name; gemm_fn fn; int smem; int ctas_per_sm; };
 static const Variant kVariants[] = {
     {"s6b2", grouped_gemm_kernel<6, 2>, smem_bytes(6), 2},     // default: two CTAs per SM, each able to saturate the DMMA pipes alone
@@ -629,8 +667,17 @@ cudaError_t gemm_kernel_setup() {
 int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf_in,
             int nrhs, long long ldx, long long ldy, bool trust_images) {
     // the tile images of x are current only if the library wrote them itself for exactly this vector (Plan::ximg_src)
-    const int skip_phase0 = (trust_images && nrhs == 1 && p->ximg_src == x) ? 1 : 0;
+    int xmode = (trust_images && nrhs == 1 && p->ximg_src == x) ? 1 : 0;
     p->ximg_src = nullptr;
+    // dmrg_davidson_step_host: x is streamed from pinned host memory (and copied to `x`)
+    XStream xs{};
+    const double *x_src = x;
+    if (p->x_stream && nrhs == 1 && p->n_xshares > 0) {
+        static const int loaders = []() { const char *e = getenv("DMRG_XLOADERS"); return e ? atoi(e) : 48; }();
+        xmode = 2; x_src = p->x_stream;
+        xs.shares = p->xshares; xs.n_shares = p->n_xshares; xs.n_loaders = std::max(1, loaders); xs.x_copy = const_cast<double *>(x);
+    }
+    p->x_stream = nullptr;
     if (nrhs < 1 || nrhs > p->max_rhs) return fail(p, DMRG_E_INVALID_ARG, "apply_H: more right-hand sides than options.max_rhs");
     BasePtrs b;
     b.p[BASE_XP] = p->ximg_p;
@@ -652,9 +699,10 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
         Prefetch pf;
         if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) pf = *pf_in;
         const int grid = (int)std::min<long long>((long long)n_units * nrhs, (long long)g_ctas_per_sm * p->sm_count);   // persistent: one wave
+        xs.n_loaders = std::min(xs.n_loaders, grid);
         g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
                                                               p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
-                                                              p->xsegs, p->n_xsegs, x, p->n, rh, skip_phase0, p->axpy);
+                                                              p->xsegs, p->n_xsegs, x_src, p->n, rh, xmode, p->axpy, xs);
     }
     if (ev) { cudaEventRecord(ev[1], st); cudaEventRecord(ev[2], st); }
     cudaError_t e = cudaGetLastError();

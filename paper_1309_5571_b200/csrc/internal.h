@@ -31,13 +31,18 @@ struct GemmItem {
     long long p_off, q_off;   // element offsets of the operands' first images in their bases
     int K;
     uint8_t p_base, q_base;
-    uint8_t pad[2];
-    int dep;                  // index of the T-block ready counter this item waits on (-1: reads no T)
-    int dep_need;             // 4 x tiles of that T block (one count per consumer warp): the counter value that means "complete"
+    uint8_t xdep;             // 1: `dep` is the ready counter of an X segment (waited on only when x is streamed in, XShare)
+    uint8_t pad;
+    int dep;                  // index of the ready counter this item waits on: a T block of this launch, or an X segment (-1: none)
+    int dep_need;             // T: 8 x tiles of that block (one count per consumer warp); X: elements of the segment
 };
 
 // Phase 0 table, one entry per segment X_ik (d_i x d_k, row-major at x + seg_off, ascending seg_off): where its P and Q images start
 struct XSeg { long long seg_off, xp_off, xq_off; int di, dk; };
+// Streamed input (dmrg_davidson_step_host with pinned host memory): a few loader CTAs pull x over PCIe share by share, in
+// the order the units need the segments, and publish the elements written per segment; the other CTAs start on the units.
+struct XShare { int seg, lo, hi, pad; };   // elements [lo, hi) of segment `seg`
+struct XStream { const XShare *shares; int n_shares, n_loaders; double *x_copy; };
 
 struct GemmUnit {
     long long c_off;          // C(0,0) in its base
@@ -62,7 +67,7 @@ struct GemmUnit {
 struct AxpyItem { long long x_off; double c; };
 
 // control words of one apply (device ints): ticket dispenser, finished count, X-image count, then one ready counter per T block
-enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_XREADY = 2, CTRL_DEP0 = 3 };   // XREADY: CTAs whose share of the X images is written
+enum Ctrl : int { CTRL_TICKET = 0, CTRL_FINISHED = 1, CTRL_XREADY = 2, CTRL_XSHARE = 3, CTRL_DEP0 = 4 };   // XREADY: CTAs whose share of the X images is written
 
 struct BasePtrs { double *p[BASE_COUNT]; };
 // Several right-hand sides in ONE grouped launch (block Davidson): ticket = unit * nrhs + rhs; every
@@ -147,7 +152,10 @@ struct Plan {
     double *pool = nullptr, *tws = nullptr, *part = nullptr, *D = nullptr;
     double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
     XSeg *xsegs = nullptr; int n_xsegs = 0;
-    AxpyItem *axpy = nullptr;
+    XShare *xshares = nullptr; int n_xshares = 0;   // streamed input: shares in the order of first use
+    int n_deps_t = 0;                               // T-block counters; the X-segment counters follow (n_deps = n_deps_t + n_xsegs)
+    const double *x_stream = nullptr;               // set for ONE apply_H: device-accessible (pinned host) source of x, streamed
+    AxpyItem *axpy = nullptr; int axpy_count = 0;
     // the vector whose tile images are current because the library itself just wrote both (dmrg_davidson_step: line 14 writes
     // the appended vector and its images); consumed by the next projection of exactly that vector inside a step, cleared by
     // every other entry point that may see a different or modified vector

@@ -15,6 +15,7 @@
 #include <cstdlib>
 #include <map>
 #include "internal.h"
+#include <climits>
 
 namespace dmrg {
 
@@ -494,10 +495,12 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
         if (r.B < 0) {            // A (x) I :  X'_jk += A X_ik
             const PoolEntry &A = bl.pool[r.A];
             it2 = {A.off, xq, (int)di, BASE_POOL, BASE_XQ};
+            it2.xdep = 1;
             flops += 2 * dj * di * dk; n_gemms += 1;
         } else if (r.A < 0) {     // I (x) B :  X'_il += X_ik B^T
             const PoolEntry &B = bl.pool[r.B];
             it2 = {xp, B.off, (int)dk, BASE_XP, BASE_POOL};
+            it2.xdep = 1;
             flops += 2 * di * dk * dl; n_gemms += 1;
         } else {
             const PoolEntry &A = bl.pool[r.A], &B = bl.pool[r.B];
@@ -521,19 +524,19 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
             }
             t1.item_begin = (int)items1.size();
             t1.out_pair = r.out_pair;
-            it1.dep = -1; it1.dep_need = 0;
+            it1.xdep = 1; it1.dep = r.in_pair; it1.dep_need = (int)(di * dk);     // counters: X segments first, T blocks after
             dep = (int)tasks1.size();
             items1.push_back(it1);
             tasks1.push_back(t1);
         }
-        it2.dep = dep;
-        it2.dep_need = dep < 0 ? 0 : CWARPS * ((tasks1[dep].M + BM - 1) / BM) * ((tasks1[dep].N + BN - 1) / BN);   // one count per consumer warp
+        if (it2.xdep) { it2.dep = r.in_pair; it2.dep_need = (int)(di * dk); }
+        else { it2.dep = P + dep; it2.dep_need = CWARPS * ((tasks1[dep].M + BM - 1) / BM) * ((tasks1[dep].N + BN - 1) / BN); }   // one count per consumer warp
         out_items[r.out_pair].push_back(it2);
     }
     // inside one output the records that read X directly come first in the K order, so that a stage-2 unit
     // starting at k = 0 has work before its first T block is complete (order fixed at plan time: deterministic)
     for (auto &v : out_items)
-        std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return (a.dep < 0) > (b.dep < 0); });
+        std::stable_sort(v.begin(), v.end(), [](const GemmItem &a, const GemmItem &b) { return a.xdep > b.xdep; });
     std::vector<AxpyItem> axpy;
     for (int op = 0; op < P; op++) {
         if (p->opt.shard_count > 1 && p->owner[op] != p->opt.shard_rank) continue;    // not ours: y segment left untouched
@@ -611,7 +614,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
                     u.kt_begin = begin; u.kt_count = base + (sp < rem ? 1 : 0); begin += u.kt_count;
                     u.tile_id = tile_id; u.split_idx = sp; u.n_split = ns;
                     u.c_base = t.c_base; u.c_kind = t.c_kind; u.c_vec2 = vec2(t.c_off, t.ldc);
-                    u.signal = signals ? (int)ti : -1;
+                    u.signal = signals ? P + (int)ti : -1;
                     u.cost = u.kt_count * (4 * sub + 64);
                     u.axpy_begin = t.axpy_begin; u.axpy_count = t.axpy_count;
                     {   // resolve kt_begin to (item, k offset) here, so that the kernel does not walk the item list
@@ -660,7 +663,26 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     }
     std::vector<GemmItem> items(items1);
     items.insert(items.end(), items2.begin(), items2.end());
-    p->n_deps = (int)tasks1.size();
+    p->n_deps_t = (int)tasks1.size();
+    p->n_deps = P + p->n_deps_t;
+    // streamed input: shares of <= 3456 elements inside one segment, segments in the order the units first need them
+    std::vector<XShare> xshares;
+    {
+        std::vector<int> first(P, INT_MAX);
+        for (size_t q = 0; q < units.size(); q++)
+            for (int e = 0; e < units[q].item_count; e++) {
+                const GemmItem &it = items[units[q].item_begin + e];
+                if (it.xdep) first[it.dep] = std::min(first[it.dep], (int)q);
+            }
+        std::vector<int> ord(P);
+        for (int op = 0; op < P; op++) ord[op] = op;
+        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return first[a] < first[b]; });
+        const int chunk = 288 * 12;
+        for (int op : ord) {
+            const long long ne = (long long)xsegs[op].di * xsegs[op].dk;
+            for (long long lo = 0; lo < ne; lo += chunk) xshares.push_back({op, (int)lo, (int)std::min<long long>(ne, lo + chunk), 0});
+        }
+    }
 
     // ---- device allocations
     CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
@@ -677,11 +699,15 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     CUDA_TRY(p, dev_alloc(p, &p->xsegs, (long long)xsegs.size()));
     if (!xsegs.empty()) CUDA_TRY(p, cudaMemcpy(p->xsegs, xsegs.data(), xsegs.size() * sizeof(XSeg), cudaMemcpyHostToDevice));
     p->n_xsegs = (int)xsegs.size();
+    CUDA_TRY(p, dev_alloc(p, &p->xshares, (long long)xshares.size()));
+    if (!xshares.empty()) CUDA_TRY(p, cudaMemcpy(p->xshares, xshares.data(), xshares.size() * sizeof(XShare), cudaMemcpyHostToDevice));
+    p->n_xshares = (int)xshares.size();
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
     CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
     CUDA_TRY(p, dev_alloc(p, &p->axpy, (long long)axpy.size()));
+    p->axpy_count = (int)axpy.size();
     if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
     CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + (long long)p->n_deps * R));
     CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
@@ -775,7 +801,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
 void plan_free(Plan *p) {
     if (!p) return;
     cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
-    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs); cudaFree(p->axpy);
+    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs); cudaFree(p->xshares); cudaFree(p->axpy);
     cudaFree(p->items); cudaFree(p->units); cudaFree(p->ctrl); cudaFree(p->trace);
     cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
     cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);

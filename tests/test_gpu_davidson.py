@@ -340,18 +340,22 @@ def test_enqueued_steps_equal_synchronous_steps(lib):
     plan.close()
 
 
-def test_step_host_equals_step_with_manual_copies(lib):
-    """dmrg_davidson_step_host (H2D of V(:,k-1) before line 2, D2H of W(:,k-1) on a side stream overlapping lines
-    3-13) must give bitwise the results of dmrg_davidson_step + the two copies done by hand, across restart steps
-    (k == k_max, where the collapse rewrites W) and with either host pointer NULL."""
+@pytest.mark.parametrize("pinned", [True, False])
+def test_step_host_equals_step_with_manual_copies(lib, pinned):
+    """dmrg_davidson_step_host (V(:,k-1) from the host before line 2 -- pinned memory is STREAMED in by loader CTAs of the
+    projection kernel while the other CTAs already compute, pageable memory is copied first --, D2H of W(:,k-1) on a side
+    stream overlapping lines 3-13) must give bitwise the results of dmrg_davidson_step + the two copies done by hand,
+    across restart steps (k == k_max, where the collapse rewrites W) and with either host pointer NULL."""
     import torch
     p = SMALL["heis_syn_m300_ragged"]()
     plan = lib.Plan(p, k_max=4, tol=1e-12)
     n = plan.n
     Va, Wa = plan.new_basis()
     Vb, Wb = plan.new_basis()
-    hx = torch.empty(n, dtype=torch.float64).pin_memory()
-    hw = torch.empty(n, dtype=torch.float64).pin_memory()
+    hx = torch.empty(n, dtype=torch.float64)
+    hw = torch.empty(n, dtype=torch.float64)
+    if pinned:
+        hx, hw = hx.pin_memory(), hw.pin_memory()
     plan.davidson_init(Va, Wa, start_at_argmin_diag=True)
     ref = []
     k = 1
