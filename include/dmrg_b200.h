@@ -231,7 +231,12 @@ int dmrg_davidson_step_given_w(dmrg_handle_t h, double *V, double *W, int64_t ld
  * V(:,k-1) on the stream before line 2; w_out_host (n doubles, or NULL) receives W(:,k-1) =
  * H_SB V(:,k-1), copied on a plan-owned side stream as soon as the projection has finished so
  * that the transfer overlaps lines 3-13 (on a restart step the collapse waits for it).  Pinned
- * host memory is needed for the copies to be asynchronous.  Always synchronises (stream and
+ * host memory is needed for the copies to be asynchronous.  A PINNED v_in_host (cudaHostAlloc /
+ * cudaHostRegister memory, anything cudaPointerGetAttributes reports as host memory) is not copied
+ * by the copy engine at all: loader CTAs of the projection kernel read it over PCIe segment by
+ * segment, in the order the work units need the segments, write V(:,k-1) and the operand images,
+ * and the other CTAs start on the segments that have arrived (same results bit for bit; a plan of
+ * the l-1-1-r strategy and pageable memory take the plain copy).  Always synchronises (stream and
  * side stream) before returning; the other arguments and the return value are those of
  * dmrg_davidson_step.  If the run had already converged the step is a no-op and w_out_host
  * receives W(:,k-1) as it stands. */
