@@ -643,8 +643,21 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
             }
             return units[a].cost > units[b].cost;
         });
+        // Split K: the LAST slice of a tile in ticket order is its reducer and waits for the other slices.  Slices of one tile
+        // are taken within a microsecond of each other and run at different paces (the partner CTA on the SM, edge tiles), so a
+        // reducer right behind its siblings idles until the slowest of them is done (measured: 8.4 us per CTA at cfg 3).  The
+        // highest slice of every split tile is therefore held back by `lag` tickets: its siblings have then finished
+        // (cfg 3 185.0 -> 183.5 us, cfg 5a 186.3 -> 182.7; 75-150 tickets are equivalent, 300 and more lengthen the drain).
+        static const int lag = []() { const char *e = getenv("DMRG_REDUCER_LAG"); return e ? atoi(e) : 150; }();
         std::vector<GemmUnit> v; v.reserve(units.size());
-        for (int q : idx) v.push_back(units[q]);
+        std::vector<std::pair<size_t, int>> held;      // (position at which it is due, unit)
+        size_t head = 0;
+        for (int q : idx) {
+            while (head < held.size() && held[head].first <= v.size()) v.push_back(units[held[head++].second]);
+            if (lag > 0 && units[q].n_split > 1 && units[q].split_idx == units[q].n_split - 1) held.push_back({v.size() + (size_t)lag, q});
+            else v.push_back(units[q]);
+        }
+        while (head < held.size()) v.push_back(units[held[head++].second]);
         units.swap(v);
     };
     std::vector<GemmUnit> units1, units2;
