@@ -19,7 +19,8 @@ dist.init_process_group("gloo")
 local_ms = 10.0 if rank == 0 else 25.0          # the slower rank sets the job time
 local_flop = 4.0e9 if rank == 0 else 6.0e9
 ms, gfl = bench.job_throughput(local_ms, local_flop, world, dist, "cpu")
-print(json.dumps({{"rank": rank, "ms": ms, "gflops": gfl}}), flush=True)
+sys.stdout.write(json.dumps({{"rank": rank, "ms": ms, "gflops": gfl}}) + "\n")     # one write: the two ranks share a pipe
+sys.stdout.flush()
 dist.destroy_process_group()
 """
 
@@ -46,7 +47,8 @@ def test_job_throughput_world_size_2(tmp_path):
         if r.returncode == 0:
             break
     assert r.returncode == 0, r.stderr[-2000:]
-    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    # (two processes write to one pipe: tolerate two records on one line)
+    rows = [json.loads(l) for l in r.stdout.replace("}{", "}\n{").splitlines() if l.startswith("{")]
     assert len(rows) == 2
     for row in rows:
         assert row["ms"] == pytest.approx(25.0)
