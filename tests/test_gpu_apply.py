@@ -283,3 +283,42 @@ def test_reserved_basis_driver_allocates_nothing(lib):
     rc, lam, x, rho, iters = plan.lowest_eigenpair(None, start_at_argmin_diag=True)
     assert rc == lib.DMRG_OK and plan.stats()["device_bytes"] == b0
     plan.close()
+
+
+def test_soak_shapes_multi_rhs_and_streamed_input(lib, monkeypatch):
+    """40 further random shapes (seeds 1000-1039, per-side dimension up to 900) with the planner's unit size varied from 3 to 200
+    units per SM: dmrg_apply_H, dmrg_apply_H_multi with three right-hand sides, and the projected vector that
+    dmrg_davidson_step_host returns for a PINNED input (streamed in by loader CTAs) against the oracle -- the ring with stages of
+    up to three k-tiles, partial stages, one-k-tile items and the per-segment ready counters all get exercised."""
+    import torch
+    for seed in range(1000, 1040):
+        p = fuzz_problem(seed, m_max=900)
+        lay = rec.Layout(p)
+        if lay.n == 0:
+            continue
+        ups = [None, 3, 40, 200][seed % 4]
+        if ups:
+            monkeypatch.setenv("DMRG_UNITS_PER_SM", str(ups))
+        else:
+            monkeypatch.delenv("DMRG_UNITS_PER_SM", raising=False)
+        plan = lib.Plan(p, k_max=6, max_rhs=3)
+        ap = oracle_apply(p, lay)
+        x = random_vector(lay.n, 7000 + seed)
+        assert rel_maxnorm(plan.apply_H(to_dev(x)).cpu().numpy(), ap(x)) <= HPSI_RTOL, seed
+        ld = (lay.n + 15) // 16 * 16
+        X = torch.zeros((3, ld), dtype=torch.float64, device="cuda"); Y = torch.empty_like(X)
+        xs = [random_vector(lay.n, 8000 + 3 * seed + r) for r in range(3)]
+        for r in range(3):
+            X[r, :lay.n] = to_dev(xs[r])
+        plan.apply_H_multi(X, Y)
+        for r in range(3):
+            assert rel_maxnorm(Y[r, :lay.n].cpu().numpy(), ap(xs[r])) <= HPSI_RTOL, (seed, r)
+        V, W = plan.new_basis()
+        plan.davidson_init(V, W, start_at_argmin_diag=True)
+        hx = V[0, :lay.n].cpu().pin_memory(); hw = torch.empty(lay.n, dtype=torch.float64).pin_memory()
+        plan.davidson_step_host(V, W, 1, hx, hw)
+        yo = ap(hx.numpy())
+        if np.max(np.abs(yo)) > 0:
+            assert rel_maxnorm(hw.numpy(), yo) <= HPSI_RTOL, seed
+        assert torch.equal(V[0, :lay.n].cpu(), hx)
+        plan.close()
