@@ -588,32 +588,34 @@ def block_davidson_probe(lib, problem, cfg, device, st):
 
 def next_rows_probe(lib, device, fp64_peak):
     """SURVEY 8(f) NEXT-1 and NEXT-2, measured: (a) dmrg_apply_H of an l-1-1-r plan on two synthetic
-    un-enlarged blocks of m = 1024 states (dmrg_inputs.heisenberg_block_synthetic, seeds 71/72): the superblock dimension is
-    that of the LR plan of the enlarged blocks (m = 2048 per side); (b) the infinite-lattice loop dmrg_infinite_heisenberg
+    un-enlarged blocks of m = 1024 and of m = 2048 states (dmrg_inputs.heisenberg_block_synthetic, seeds 71/72): the superblock
+    dimension is that of the LR plan of the enlarged blocks (2 m per side); (b) the infinite-lattice loop dmrg_infinite_heisenberg
     (Alg. 1, every step on the device) to 64 sites with m = 128, wall clock around the C-ABI call."""
     import torch
     from dmrg_inputs import heisenberg_block_synthetic
     out = {}
-    l, r = heisenberg_block_synthetic(1024, 4, 71), heisenberg_block_synthetic(1024, 4, 72)
-    plan = lib.Plan.from_l11r(l, r, 1.0, 1.0, 0, device=device)
-    st = plan.stats()
-    x = torch.randn(plan.n, dtype=torch.float64, device=device); y = torch.empty_like(x)
     stream = torch.cuda.current_stream()
-    for _ in range(3):
-        plan.apply_H(x, y)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(10):
-        plan.apply_H(x, y)
-    e1.record(stream); torch.cuda.synchronize()
-    us = e0.elapsed_time(e1) / 10 * 1e3
-    out["l11r_apply"] = {"workload": "l-1-1-r, two synthetic blocks of m = 1024 (9 sectors), target 2 S_z = 0", "n": int(plan.n),
-                         "flop_per_apply": int(st["flop_per_apply"]), "us_per_apply": us,
-                         "tflops": st["flop_per_apply"] / (us * 1e-6) / 1e12,
-                         "frac_fp64_peak": st["flop_per_apply"] / (us * 1e-6) / 1e12 / fp64_peak,
-                         "units": int(st["stage1_units"] + st["stage2_units"])}
-    plan.close()
-    del x, y
+    for m in (1024, 2048):
+        l, r = heisenberg_block_synthetic(m, 4, 71), heisenberg_block_synthetic(m, 4, 72)
+        plan = lib.Plan.from_l11r(l, r, 1.0, 1.0, 0, device=device)
+        st = plan.stats()
+        x = torch.randn(plan.n, dtype=torch.float64, device=device); y = torch.empty_like(x)
+        for _ in range(3):
+            plan.apply_H(x, y)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(10):
+            plan.apply_H(x, y)
+        e1.record(stream); torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) / 10 * 1e3
+        out["l11r_apply" if m == 1024 else f"l11r_apply_m{m}"] = {
+            "workload": f"l-1-1-r, two synthetic blocks of m = {m} (9 sectors), target 2 S_z = 0", "n": int(plan.n),
+            "flop_per_apply": int(st["flop_per_apply"]), "us_per_apply": us,
+            "tflops": st["flop_per_apply"] / (us * 1e-6) / 1e12,
+            "frac_fp64_peak": st["flop_per_apply"] / (us * 1e-6) / 1e12 / fp64_peak,
+            "units": int(st["stage1_units"] + st["stage2_units"])}
+        plan.close()
+        del x, y
     lib.infinite_heisenberg(16, 32)                      # warm-up (module load, allocator)
     t0 = time.perf_counter()
     recs = lib.infinite_heisenberg(64, 128)

@@ -568,7 +568,12 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     // (measured: 16 is best at cfg 3 / 5a, ~280 k-tile units per SM; 24 at the 4096 sweep, 2200 per SM; flat beyond)
     long long ups = (Wtot / std::max(p->sm_count, 1) < 1000) ? 12 : 24;   // re-measured with the persistent kernel: 10-12 best at cfg 3 / 5a
     if (const char *e = getenv("DMRG_UNITS_PER_SM")) ups = std::max(1, atoi(e));
-    const long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
+    // ... but do not aim below kt_floor k-tiles per unit when there is work for it: with little work per SM (the l-1-1-r plans, small superblocks) units of
+    // two ring stages are all boundary (l-1-1-r, two blocks of m = 1024: 86 -> 76 us with units of >= 18 k-tiles)
+    long long kt_floor = 18;
+    if (const char *e = getenv("DMRG_KT_FLOOR")) kt_floor = std::max(1, atoi(e));
+    long long kt_unit = std::max<long long>(kt_min, (Wtot + (long long)p->sm_count * ups - 1) / ((long long)p->sm_count * ups));
+    if (kt_unit < kt_floor && Wtot / kt_floor >= 4LL * p->sm_count) kt_unit = kt_floor;      // (only if that still leaves two units per CTA)
     std::vector<long long> out_cost(P, 0);
     std::vector<int> unit_out, uo1, uo2;
     // "guided" unit size for stage 2: the outputs that come last in ticket order get smaller K slices (the drain of
