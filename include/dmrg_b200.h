@@ -348,6 +348,24 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *opts, int32_t max_records
 /* out[0..k) = V(:,0..k)^T w   (gemv_trans).  out DEVICE k doubles. */
 int dmrg_gemv_trans(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
                     const double *w, double *out, void *cuda_stream);
+/* dmrg_gemv_trans for callers that may not allocate (code under CUDA stream capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): out[0..k) = V(:,0..k)^T w with NO plan handle and NO allocation of any kind -- the call makes no cudaMalloc,
+ * cudaFree or allocating library call; it enqueues one 4-byte memset and one kernel on the stream.  Same kernel and arithmetic as
+ * dmrg_gemv_trans (Alg. 3 lines 3 and 12; Alg. 4); the cross-CTA scratch of that kernel (one row of partial
+ * sums per CTA, fixed-order final sum by the last CTA, and its arrival counter) lives in a file-scope device array of
+ * DMRG_STATIC_SCRATCH_BYTES bytes that every GPU which loads the library holds until the process exits.
+ *   V    DEVICE, column j at V + j*ldv, n doubles each (ldv >= n);   w  DEVICE, n doubles;   out  DEVICE, k doubles, overwritten.
+ *   Limits: 1 <= k <= DMRG_STATIC_MAX_K, 1 <= n <= DMRG_STATIC_MAX_N; anything beyond is DMRG_E_INVALID_ARG with a message
+ *   (dmrg_last_error(NULL)), nothing is launched.  The grid is at most 1024 CTAs (the rows of the scratch), so n does not size it.
+ *   The current device is used; asynchronous on `cuda_stream`; V, w, out are the caller's and are not retained.
+ *   ALL calls on a device share the one scratch array, which keeps the last call's contents (every call rewrites the partial sums
+ *   it reads and clears the counter): calls that may OVERLAP on the GPU -- different streams without an ordering between them --
+ *   race on it and give wrong results.  Calls on one stream, or ordered by events, are safe.  It does not interfere with plans. */
+#define DMRG_STATIC_MAX_K 32
+#define DMRG_STATIC_MAX_N (((int64_t)1) << 40)
+#define DMRG_STATIC_SCRATCH_BYTES 278784
+int dmrg_gemv_trans_static(const double *V, int64_t ldv, int64_t n, int32_t k, const double *w, double *out,
+                           void *cuda_stream);
 /* t -= V(:,0..k) s  and  *nrm2_out = ||t||^2 (gemv). s, nrm2_out DEVICE. */
 int dmrg_gemv_sub(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k,
                   const double *s, double *t, double *nrm2_out, void *cuda_stream);

@@ -28,6 +28,7 @@ EXPORTS = [
     "dmrg_block_lowest_eigenpairs",
     "dmrg_plan_create_l11r", "dmrg_partition_outputs", "dmrg_get_shard", "dmrg_davidson_step_given_w",
     "dmrg_density_matrix", "dmrg_sector_eig", "dmrg_select_states", "dmrg_rotate_op", "dmrg_infinite_heisenberg",
+    "dmrg_gemv_trans_static",
 ]
 
 
@@ -115,6 +116,7 @@ def load_library():
         "dmrg_ritz_vector": [vp, vp, i64, i32, vp, vp],
         "dmrg_lowest_eigenpair": [vp, vp, i32, vp, pdbl, pdbl, pi32, vp],
         "dmrg_gemv_trans": [vp, vp, i64, i32, vp, vp, vp],
+        "dmrg_gemv_trans_static": [vp, i64, i64, i32, vp, vp, vp],
         "dmrg_gemv_sub": [vp, vp, i64, i32, vp, vp, vp, vp],
         "dmrg_probe_fp64_peak": [i32, i32, pdbl, vp],
         "dmrg_probe_hbm_read": [i64, i32, pdbl, vp],
@@ -198,6 +200,29 @@ def infinite_heisenberg(n_sites: int, m_keep: int, J: float = 1.0, Delta: float 
         raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
     return [dict(n_sites=int(ns[q]), energy=float(e[q]), discarded=(float(dl[q]), float(dr[q])), n=int(td[q]), davidson_iters=int(it[q]))
             for q in range(nr.value)]
+
+
+def gemv_trans_static(V, k: int, w, out, n: Optional[int] = None, stream=None):
+    """dmrg_gemv_trans_static: out[0..k) = V(:,0..k)^T w without a plan and without any allocation (scratch in a file-scope device
+    array; k <= 32; calls that overlap on the GPU race).  V: (>= k, ldv) or flat float64 CUDA tensor, rows = basis vectors; w: n
+    doubles; out: k doubles, caller-allocated (this wrapper allocates nothing either)."""
+    torch = _torch()
+    lib = load_library()
+    n = int(w.numel() if n is None else n)
+    for t, name in ((V, "V"), (w, "w"), (out, "out")):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
+            raise TypeError(f"{name}: need a float64 CUDA tensor")
+    if V.dim() == 2 and V.stride(1) != 1 or not w.is_contiguous() or not out.is_contiguous():
+        raise TypeError("gemv_trans_static: rows of V, w and out must be contiguous")
+    ldv = V.stride(0) if V.dim() == 2 else n
+    rows = V.shape[0] if V.dim() == 2 else V.numel() // max(n, 1)
+    if 1 <= k <= 32 and (rows < k or out.numel() < k or w.numel() < n or (V.dim() == 2 and V.shape[1] < n)):
+        raise ValueError("gemv_trans_static: V, w or out smaller than (k, n) asks for")
+    rc = lib.dmrg_gemv_trans_static(C.c_void_p(_ptr(V)), C.c_int64(int(ldv)), C.c_int64(n), C.c_int32(int(k)), C.c_void_p(_ptr(w)),
+                                    C.c_void_p(_ptr(out)), C.c_void_p(_stream_ptr(stream)))
+    if rc != DMRG_OK:
+        raise DmrgError(rc, (lib.dmrg_last_error(None) or b"").decode())
+    return out
 
 
 def _torch():

@@ -422,6 +422,10 @@ int dmrg_gemv_trans(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, co
     return dav_gemv_trans(P(h), V, ldv, k, w, out, S(stream));
 }
 
+int dmrg_gemv_trans_static(const double *V, int64_t ldv, int64_t n, int32_t k, const double *w, double *out, void *stream) {
+    return dav_gemv_trans_static(V, ldv, n, k, w, out, S(stream));
+}
+
 int dmrg_gemv_sub(dmrg_handle_t h, const double *V, int64_t ldv, int32_t k, const double *s, double *t,
                   double *nrm2_out, void *stream) {
     if (!h || !V || !s || !t || !nrm2_out) return DMRG_E_INVALID_ARG;

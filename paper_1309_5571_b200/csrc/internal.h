@@ -224,6 +224,8 @@ int dav_gemv_sub(Plan *p, const double *V, long long ldv, int k, const double *s
 // Optional side job of the last CTAs of an apply: pull the first `rows` rows of `cols` columns (column stride `ld`)
 // into L2 for the kernel that follows (the Davidson basis for line 3), while the launch drains and HBM is idle.
 struct Prefetch { const double *base = nullptr; long long ld = 0, rows = 0; int cols = 0, first_ticket = 0, n_ctas = 0; };
+// davidson.cu: dmrg_gemv_trans_static (no plan, no allocation: scratch in a file-scope device array)
+int dav_gemv_trans_static(const double *V, long long ldv, long long n, int k, const double *w, double *out, cudaStream_t st);
 int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStream_t st, const Prefetch *pf = nullptr,
             int nrhs = 1, long long ldx = 0, long long ldy = 0, bool trust_images = false);
 
