@@ -162,6 +162,9 @@ struct Plan {
     const double *ximg_src = nullptr;
     int *counters = nullptr;
     GemmItem *items = nullptr;          // stage-1 items, then stage-2 items
+    void *arena = nullptr;              // the ONE device allocation of the plan; every buffer below is a slice of it (plan.cu)
+    std::vector<std::pair<void **, size_t>> arena_reqs;
+    bool own_basis_in_arena = false;
     GemmUnit *units = nullptr;          // ticket order: stage-1 units, then stage-2 units
     int n_units1 = 0, n_units2 = 0, n_deps = 0;
     int *ctrl = nullptr;                // Ctrl layout, self-resetting

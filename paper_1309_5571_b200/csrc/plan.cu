@@ -14,8 +14,10 @@
 #include <cstring>
 #include <cstdlib>
 #include <map>
+#include <mutex>
 #include "internal.h"
 #include <climits>
+#include <time.h>
 
 namespace dmrg {
 
@@ -180,13 +182,45 @@ void partition_outputs(int n_outputs, const long long *cost, int n_ranks, int *o
 
 template <class T>
 static cudaError_t dev_alloc(Plan *p, T **ptr, long long count) {
-    size_t bytes = (size_t)std::max<long long>(count, 1) * sizeof(T);
-    cudaError_t e = cudaMalloc((void **)ptr, bytes);
-    if (e == cudaSuccess) p->device_bytes += (long long)bytes;
-    return e;
+    // One device allocation per plan: the buffers are RESERVED here (256-byte aligned slices of one arena) and get their
+    // addresses in arena_commit -- a plan is created per superblock, and two dozen cudaMalloc / cudaFree pairs were a third of
+    // the time of plan creation + destruction (8.6 + 3.2 ms at cfg 3).
+    const size_t bytes = ((size_t)std::max<long long>(count, 1) * sizeof(T) + 255) & ~(size_t)255;
+    *ptr = nullptr;
+    p->arena_reqs.push_back({reinterpret_cast<void **>(ptr), bytes});
+    p->device_bytes += (long long)bytes;
+    return cudaSuccess;
+}
+static cudaError_t arena_commit(Plan *p) {
+    size_t total = 0;
+    for (auto &r : p->arena_reqs) total += r.second;
+    cudaError_t e = cudaMalloc(&p->arena, std::max<size_t>(total, 256));
+    if (e != cudaSuccess) return e;
+    char *base = static_cast<char *>(p->arena);
+    for (auto &r : p->arena_reqs) { *r.first = base; base += r.second; }
+    p->arena_reqs.clear();
+    return cudaSuccess;
+}
+// pinned host copies of the Davidson state are recycled across plans (cudaMallocHost costs ~1 ms)
+static std::mutex g_state_mu;
+static std::vector<DavState *> g_state_free;
+static cudaError_t state_host_get(DavState **out) {
+    {
+        std::lock_guard<std::mutex> lk(g_state_mu);
+        if (!g_state_free.empty()) { *out = g_state_free.back(); g_state_free.pop_back(); return cudaSuccess; }
+    }
+    return cudaHostAlloc((void **)out, sizeof(DavState), cudaHostAllocPortable);
+}
+static void state_host_put(DavState *s) {
+    if (!s) return;
+    std::lock_guard<std::mutex> lk(g_state_mu);
+    if (g_state_free.size() < 8) g_state_free.push_back(s); else cudaFreeHost(s);
 }
 
+static double now_ms() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; }
+#define TCK(lab) do { if (tdbg) { double t = now_ms(); fprintf(stderr, "  plan %-28s %.3f ms\n", lab, t - tlast); tlast = t; } } while (0)
 int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, const dmrg_problem_l11r *l11) {
+    const bool tdbg = getenv("DMRG_PLAN_TIMING") != nullptr; double tlast = now_ms();
     *out = nullptr;
     if (!pr) return fail(nullptr, DMRG_E_INVALID_ARG, "problem is NULL");
     if (pr->model != DMRG_HEISENBERG && pr->model != DMRG_HUBBARD)
@@ -230,12 +264,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     for (int d : p->dimR) if (d < 0) { delete p; return fail(nullptr, DMRG_E_SECTOR, "negative sector dimension"); }
 
     {   // device properties
-        int dev = 0; cudaDeviceProp prop;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        int dev = 0, sms = 0;      // (one attribute, not cudaGetDeviceProperties: that call alone takes over a millisecond)
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+            cudaGetLastError();
             delete p; return fail(nullptr, DMRG_E_CUDA, "no CUDA device: this library has no CPU fallback");
         }
-        p->sm_count = prop.multiProcessorCount;
+        p->sm_count = sms;
     }
+    TCK("arguments + device query");
 
     // ---- operator validation (A4, A26)
     struct Chk { const char *nm; const dmrg_block_op *op; bool left; bool diag; };
@@ -703,38 +739,56 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     }
 
     // ---- device allocations
-    CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
     // per-apply buffers and counters exist once per right-hand side (options.max_rhs; block Davidson)
     const int R = p->max_rhs;
     p->tws_elems = tws_elems; p->part_elems = part_elems; p->xp_elems = xp_elems; p->xq_elems = xq_elems; p->n_counters = n_counters;
     tws_elems *= R; part_elems *= R; xp_elems *= R; xq_elems *= R; n_counters *= R;
+    p->vec_grid = p->sm_count * 8;      // capacity of the partials buffer; each kernel launches one wave of its own (davidson.cu)
+    p->n_xsegs = (int)xsegs.size(); p->n_xshares = (int)xshares.size(); p->axpy_count = (int)axpy.size();
+    TCK("records, units (host)");
+    // (1) every buffer is reserved, (2) one allocation, (3) initial contents
+    CUDA_TRY(p, dev_alloc(p, &p->pool, bl.pool_elems));
     CUDA_TRY(p, dev_alloc(p, &p->tws, tws_elems));
     CUDA_TRY(p, dev_alloc(p, &p->part, part_elems));
     CUDA_TRY(p, dev_alloc(p, &p->ximg_p, xp_elems));
     CUDA_TRY(p, dev_alloc(p, &p->ximg_q, xq_elems));
-    CUDA_TRY(p, cudaMemset(p->ximg_p, 0, sizeof(double) * std::max<long long>(xp_elems, 1)));   // the pads stay zero for good
-    CUDA_TRY(p, cudaMemset(p->ximg_q, 0, sizeof(double) * std::max<long long>(xq_elems, 1)));
     CUDA_TRY(p, dev_alloc(p, &p->xsegs, (long long)xsegs.size()));
-    if (!xsegs.empty()) CUDA_TRY(p, cudaMemcpy(p->xsegs, xsegs.data(), xsegs.size() * sizeof(XSeg), cudaMemcpyHostToDevice));
-    p->n_xsegs = (int)xsegs.size();
     CUDA_TRY(p, dev_alloc(p, &p->xshares, (long long)xshares.size()));
-    if (!xshares.empty()) CUDA_TRY(p, cudaMemcpy(p->xshares, xshares.data(), xshares.size() * sizeof(XShare), cudaMemcpyHostToDevice));
-    p->n_xshares = (int)xshares.size();
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
     CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
     CUDA_TRY(p, dev_alloc(p, &p->axpy, (long long)axpy.size()));
-    p->axpy_count = (int)axpy.size();
-    if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
     CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + (long long)p->n_deps * R));
-    CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
     if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
         // 4 words per unit, then 4 words per CTA (phase stamps: entry, X images written, producer released, exit)
         p->trace_units = (int)units.size() * R + 8 * p->sm_count;
         CUDA_TRY(p, dev_alloc(p, &p->trace, 4LL * std::max<long long>(p->trace_units, 1)));
-        CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     }
+    CUDA_TRY(p, dev_alloc(p, &p->state, 1));            // Davidson scratch
+    CUDA_TRY(p, dev_alloc(p, &p->tvec, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->xs, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->ws, p->n));
+    CUDA_TRY(p, dev_alloc(p, &p->partials, (long long)p->vec_grid * (KMAX + 2)));
+    CUDA_TRY(p, dev_alloc(p, &p->vec_counter, 4));
+    if (p->opt.reserve_basis) {                          // the drivers' own basis
+        p->ldv_own = (p->n + 15) / 16 * 16;
+        CUDA_TRY(p, dev_alloc(p, &p->Vown, p->ldv_own * p->opt.k_max));
+        CUDA_TRY(p, dev_alloc(p, &p->Wown, p->ldv_own * p->opt.k_max));
+        p->own_basis_in_arena = true;
+    }
+    {
+        cudaError_t ea = arena_commit(p);
+        if (ea != cudaSuccess) { std::string m = std::string("device allocation of the plan: ") + cudaGetErrorString(ea); plan_free(p); return fail(nullptr, ea == cudaErrorMemoryAllocation ? DMRG_E_ALLOC : DMRG_E_CUDA, m); }
+    }
+    TCK("arena cudaMalloc");
+    CUDA_TRY(p, cudaMemset(p->ximg_p, 0, sizeof(double) * std::max<long long>(xp_elems, 1)));   // the pads stay zero for good
+    CUDA_TRY(p, cudaMemset(p->ximg_q, 0, sizeof(double) * std::max<long long>(xq_elems, 1)));
+    if (!xsegs.empty()) CUDA_TRY(p, cudaMemcpy(p->xsegs, xsegs.data(), xsegs.size() * sizeof(XSeg), cudaMemcpyHostToDevice));
+    if (!xshares.empty()) CUDA_TRY(p, cudaMemcpy(p->xshares, xshares.data(), xshares.size() * sizeof(XShare), cudaMemcpyHostToDevice));
+    if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
+    CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
+    if (p->trace) CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     CUDA_TRY(p, cudaMemset(p->pool, 0, sizeof(double) * std::max<long long>(bl.pool_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->tws, 0, sizeof(double) * std::max<long long>(tws_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->counters, 0, sizeof(int) * std::max(n_counters, 1)));
@@ -742,7 +796,12 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     if (!items.empty()) CUDA_TRY(p, cudaMemcpy(p->items, items.data(), items.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
     if (!units.empty()) CUDA_TRY(p, cudaMemcpy(p->units, units.data(), units.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
     p->n_units1 = (int)units1.size(); p->n_units2 = (int)units2.size();
+    CUDA_TRY(p, cudaMemset(p->state, 0, sizeof(DavState)));
+    CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
+    CUDA_TRY(p, state_host_get(&p->state_host));
+    memset(p->state_host, 0, sizeof(DavState));
 
+    TCK("memsets + table copies");
     // ---- repack the operators (scaled / transposed / aligned), once
     for (const RepackJob &j : bl.jobs) {
         if (j.rows == 0 || j.cols == 0) continue;
@@ -751,6 +810,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     }
     CUDA_TRY(p, cudaGetLastError());
 
+    TCK("repack launches");
     // ---- diag(H_SB) (A14): records with (i,k) == (j,l)
     for (const Record &r : all_recs) {
         if (r.in_pair != r.out_pair) continue;
@@ -773,33 +833,23 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
         }
     CUDA_TRY(p, cudaGetLastError());
 
+    TCK("diag launches");
     // ---- Davidson scratch
-    p->vec_grid = p->sm_count * 8;      // capacity of the partials buffer; each kernel launches one wave of its own (davidson.cu)
-    CUDA_TRY(p, dev_alloc(p, &p->state, 1));
-    CUDA_TRY(p, cudaMemset(p->state, 0, sizeof(DavState)));
-    CUDA_TRY(p, cudaMallocHost((void **)&p->state_host, sizeof(DavState)));
-    memset(p->state_host, 0, sizeof(DavState));
-    CUDA_TRY(p, dev_alloc(p, &p->tvec, p->n));
-    CUDA_TRY(p, dev_alloc(p, &p->xs, p->n));
-    CUDA_TRY(p, dev_alloc(p, &p->ws, p->n));
-    CUDA_TRY(p, dev_alloc(p, &p->partials, (long long)p->vec_grid * (KMAX + 2)));
-    CUDA_TRY(p, dev_alloc(p, &p->vec_counter, 4));
-    CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
+    TCK("davidson scratch alloc");
     CUDA_TRY(p, gemm_kernel_setup());
+    TCK("gemm_kernel_setup");
     dav_setup(p);
+    TCK("dav_setup");
     // everything a hot call needs exists from here on: side stream and events of dmrg_davidson_step_host, the ordering
     // event, and (options.reserve_basis) the drivers' own basis
     CUDA_TRY(p, cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking));
     CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_apply, cudaEventDisableTiming));
     CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming));
     CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_last, cudaEventDisableTiming));
-    if (p->opt.reserve_basis) {
-        p->ldv_own = (p->n + 15) / 16 * 16;
-        CUDA_TRY(p, dev_alloc(p, &p->Vown, p->ldv_own * p->opt.k_max));
-        CUDA_TRY(p, dev_alloc(p, &p->Wown, p->ldv_own * p->opt.k_max));
-    }
     { int rcb = block_alloc(p); if (rcb != DMRG_OK) { std::string m = p->err; plan_free(p); return fail(nullptr, rcb, m); } }
+    TCK("stream/events/block_alloc");
     CUDA_TRY(p, cudaDeviceSynchronize());
+    TCK("device synchronize");
 
     // ---- stats
     dmrg_stats &s = p->stats;
@@ -818,12 +868,9 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
 
 void plan_free(Plan *p) {
     if (!p) return;
-    cudaFree(p->pool); cudaFree(p->tws); cudaFree(p->part); cudaFree(p->counters); cudaFree(p->D);
-    cudaFree(p->ximg_p); cudaFree(p->ximg_q); cudaFree(p->xsegs); cudaFree(p->xshares); cudaFree(p->axpy);
-    cudaFree(p->items); cudaFree(p->units); cudaFree(p->ctrl); cudaFree(p->trace);
-    cudaFree(p->state); if (p->state_host) cudaFreeHost(p->state_host);
-    cudaFree(p->tvec); cudaFree(p->xs); cudaFree(p->ws); cudaFree(p->partials); cudaFree(p->vec_counter);
-    cudaFree(p->Vown); cudaFree(p->Wown);
+    cudaFree(p->arena);                                  // every plan buffer is a slice of it
+    state_host_put(p->state_host);
+    if (!p->own_basis_in_arena) { cudaFree(p->Vown); cudaFree(p->Wown); }      // (allocated later by a driver: api.cu)
     block_free(p);
     if (p->timing.created) for (auto &e : p->timing.ev) cudaEventDestroy(e);
     if (p->ev_apply) cudaEventDestroy(p->ev_apply);

@@ -11,6 +11,8 @@
 #include <cstring>
 #include <map>
 #include <vector>
+#include <time.h>
+#include <cstdio>
 #include "internal.h"
 
 namespace dmrg {
@@ -134,19 +136,31 @@ __device__ __forceinline__ void rot_pair(double app, double aqq, double apq, dou
 }
 __global__ void __launch_bounds__(ET)
 sector_eig_kernel(const EigJob *__restrict__ jobs, double *__restrict__ Aall, double *__restrict__ Eall, double *__restrict__ Uall,
-                  double *__restrict__ wall, int *__restrict__ status) {
+                  double *__restrict__ wall, int *__restrict__ status, int hdr_half, long long mat_doubles) {
     extern __shared__ unsigned char eig_smem[];
     const EigJob jb = jobs[blockIdx.x];
     const int d = jb.d, tid = threadIdx.x;
     if (d == 0) return;
     double *A = Aall + jb.off, *E = Eall + jb.off, *U = Uall + jb.off, *w = wall + jb.w_off;
     const int n = (d + 1) & ~1, half = n / 2;
-    double *s_c = reinterpret_cast<double *>(eig_smem);          // [half]
-    double *s_s = s_c + half;                                    // [half]
-    int *s_p = reinterpret_cast<int *>(s_s + half);              // [half]
-    int *s_q = s_p + half;                                       // [half]
+    double *s_c = reinterpret_cast<double *>(eig_smem);          // [hdr_half]
+    double *s_s = s_c + hdr_half;                                // [hdr_half]
+    int *s_p = reinterpret_cast<int *>(s_s + hdr_half);          // [hdr_half]
+    int *s_q = s_p + hdr_half;                                   // [hdr_half]
     __shared__ double s_red[2][ET / 32];
     __shared__ int s_stop;
+    // The sweeps read and write every element of A and E 3 (n - 1) times with a CTA barrier in between: out of global memory a
+    // round is three L2 round trips (~9 us at d = 190).  When they fit, A -- and E too -- live in shared memory for the whole
+    // solve (mat_doubles doubles were allocated behind the header): d <= 118 both, d <= 167 A alone.
+    {
+        double *mat = reinterpret_cast<double *>(s_q + hdr_half);      // 24 hdr_half bytes in: 8-byte aligned
+        const long long dd = (long long)d * d;
+        if (dd <= mat_doubles) {
+            for (long long e = tid; e < dd; e += ET) mat[e] = A[e];
+            A = mat;
+            if (2 * dd <= mat_doubles) E = mat + dd;
+        }
+    }
     for (long long e = tid; e < (long long)d * d; e += ET) E[e] = (e / d == e % d) ? 1.0 : 0.0;
     __syncthreads();
     int sweep = 0;
@@ -267,10 +281,15 @@ int sector_eig(int ns, const int *dims, double *rho, double *U, double *w, cudaS
     DevBuf<EigJob> dj; DevBuf<double> E; DevBuf<int> status;
     RN_TRY(dj.upload(jobs, st)); RN_TRY(E.alloc((size_t)off)); RN_TRY(status.alloc(1, true));
     const int half = ((dmax + 1) & ~1) / 2;
-    const size_t smem = (size_t)half * (2 * sizeof(double) + 2 * sizeof(int));
-    if (smem > 200 * 1024) return fail(nullptr, DMRG_E_INVALID_ARG, "sector_eig: a sector larger than 12800 states");
+    const size_t hdr = (size_t)(half + (half & 1)) * (2 * sizeof(double) + 2 * sizeof(int));
+    if (hdr > 200 * 1024) return fail(nullptr, DMRG_E_INVALID_ARG, "sector_eig: a sector larger than 12800 states");
+    // shared memory behind the header for the matrices of the largest sector (both if they fit, else A alone, else none)
+    const size_t cap = (size_t)225 * 1024 - hdr;
+    const size_t dd = (size_t)dmax * dmax * sizeof(double);
+    const size_t mat_bytes = 2 * dd <= cap ? 2 * dd : (dd <= cap ? dd : 0);
+    const size_t smem = hdr + mat_bytes;
     RN_TRY(cudaFuncSetAttribute(sector_eig_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024)));
-    if (ns > 0) sector_eig_kernel<<<ns, ET, smem, st>>>(dj.p, rho, E.p, U, w, status.p);
+    if (ns > 0) sector_eig_kernel<<<ns, ET, smem, st>>>(dj.p, rho, E.p, U, w, status.p, half, (long long)(mat_bytes / sizeof(double)));
     RN_TRY(cudaGetLastError());
     int hs = 0;
     RN_TRY(cudaMemcpyAsync(&hs, status.p, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -411,33 +430,55 @@ int enlarge(const DevBlock &b, int side, double J, double Delta, DevBlock &e, cu
 // ---------------------------------------------------------------- Alg. 1 looped: infinite-lattice DMRG, Heisenberg chain
 namespace {
 
-int renormalise_side(Plan *p, const DevBlock &b, int side, const double *x, int m, DevBlock &out, double *discarded, cudaStream_t st) {
-    const int ns = (int)b.dims.size();
-    long long tot = 0, wtot = 0;
-    for (int d : b.dims) { tot += (long long)d * d; wtot += d; }
+static double g_t[8];
+static double rn_now() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; }
+#define RNT(i, st_) do { if (g_tdbg) { cudaStreamSynchronize(st_); double t_ = rn_now(); g_t[i] += t_ - g_tl; g_tl = t_; } } while (0)
+static bool g_tdbg = false; static double g_tl = 0;
+// Alg. 1 lines 4-7 for BOTH blocks of the superblock: the density matrices of the two sides, then ONE eigen-solver launch over
+// the sectors of both (the launch lasts as long as its largest sector: two launches would take twice as long), then the choice of
+// states and the rotations side by side.
+int renormalise_both(Plan *p, const DevBlock &bl, const DevBlock &br, const double *x, int m, DevBlock &outl, DevBlock &outr,
+                     double *disc_l, double *disc_r, cudaStream_t st) {
+    const DevBlock *bs[2] = {&bl, &br};
+    DevBlock *outs[2] = {&outl, &outr};
+    double *disc[2] = {disc_l, disc_r};
+    long long tot[2] = {0, 0}, wtot[2] = {0, 0};
+    std::vector<int> dims_all;
+    for (int side = 0; side < 2; side++)
+        for (int d : bs[side]->dims) { tot[side] += (long long)d * d; wtot[side] += d; dims_all.push_back(d); }
     DevBuf<double> rho, U, w;
-    RN_TRY(rho.alloc((size_t)tot)); RN_TRY(U.alloc((size_t)tot)); RN_TRY(w.alloc((size_t)wtot));
-    int rc = density_matrix(p, x, side, rho.p, st);                          // line 5
-    if (rc == DMRG_OK) rc = sector_eig(ns, b.dims.data(), rho.p, U.p, w.p, st);   // line 6
+    RN_TRY(rho.alloc((size_t)(tot[0] + tot[1]))); RN_TRY(U.alloc((size_t)(tot[0] + tot[1]))); RN_TRY(w.alloc((size_t)(wtot[0] + wtot[1])));
+    RNT(3, st);
+    int rc = density_matrix(p, x, 0, rho.p, st);                                       // line 5
+    if (rc == DMRG_OK) rc = density_matrix(p, x, 1, rho.p + tot[0], st);
+    RNT(4, st);
+    if (rc == DMRG_OK) rc = sector_eig((int)dims_all.size(), dims_all.data(), rho.p, U.p, w.p, st);      // line 6
+    RNT(5, st);
     if (rc != DMRG_OK) return rc;
-    std::vector<double> wh((size_t)wtot);
-    RN_TRY(cudaMemcpyAsync(wh.data(), w.p, sizeof(double) * (size_t)wtot, cudaMemcpyDeviceToHost, st));
+    std::vector<double> wh((size_t)(wtot[0] + wtot[1]));
+    RN_TRY(cudaMemcpyAsync(wh.data(), w.p, sizeof(double) * wh.size(), cudaMemcpyDeviceToHost, st));
     RN_TRY(cudaStreamSynchronize(st));
-    std::vector<int> keep(ns);
-    select_states(ns, b.dims.data(), wh.data(), m, keep.data(), discarded);  // line 7: which states
-    out.labels = b.labels; out.dims = keep; out.n_sites = b.n_sites;
-    for (int which = 0; which < 3; which++) {                                // line 7: rotate H, Sz, Sp
-        const DevOp &o = which == 0 ? b.H : (which == 1 ? b.Sz : b.Sp);
-        DevOp &r = which == 0 ? out.H : (which == 1 ? out.Sz : out.Sp);
-        const int nb = (int)o.src.size();
-        std::vector<long long> ooff(nb); long long elems = 0;
-        rc = rotate_op(ns, b.dims.data(), keep.data(), U.p, nb, o.src.data(), o.dst.data(), o.off.data(), o.ld.data(), o.data.p, nullptr, ooff.data(), &elems, st);
-        if (rc != DMRG_OK) return rc;
-        RN_TRY(r.data.alloc((size_t)elems));
-        rc = rotate_op(ns, b.dims.data(), keep.data(), U.p, nb, o.src.data(), o.dst.data(), o.off.data(), o.ld.data(), o.data.p, r.data.p, ooff.data(), &elems, st);
-        if (rc != DMRG_OK) return rc;
-        for (int q = 0; q < nb; q++) if (ooff[q] >= 0) { r.add(o.src[q], o.dst[q], keep[o.dst[q]], keep[o.src[q]]); }
+    for (int side = 0; side < 2; side++) {
+        const DevBlock &b = *bs[side]; DevBlock &out = *outs[side];
+        const int ns = (int)b.dims.size();
+        const double *Us = U.p + (side ? tot[0] : 0);
+        std::vector<int> keep(ns);
+        select_states(ns, b.dims.data(), wh.data() + (side ? wtot[0] : 0), m, keep.data(), disc[side]);  // line 7: which states
+        out.labels = b.labels; out.dims = keep; out.n_sites = b.n_sites;
+        for (int which = 0; which < 3; which++) {                                // line 7: rotate H, Sz, Sp
+            const DevOp &o = which == 0 ? b.H : (which == 1 ? b.Sz : b.Sp);
+            DevOp &r = which == 0 ? out.H : (which == 1 ? out.Sz : out.Sp);
+            const int nb = (int)o.src.size();
+            std::vector<long long> ooff(nb); long long elems = 0;
+            rc = rotate_op(ns, b.dims.data(), keep.data(), Us, nb, o.src.data(), o.dst.data(), o.off.data(), o.ld.data(), o.data.p, nullptr, ooff.data(), &elems, st);
+            if (rc != DMRG_OK) return rc;
+            RN_TRY(r.data.alloc((size_t)elems));
+            rc = rotate_op(ns, b.dims.data(), keep.data(), Us, nb, o.src.data(), o.dst.data(), o.off.data(), o.ld.data(), o.data.p, r.data.p, ooff.data(), &elems, st);
+            if (rc != DMRG_OK) return rc;
+            for (int q = 0; q < nb; q++) if (ooff[q] >= 0) { r.add(o.src[q], o.dst[q], keep[o.dst[q]], keep[o.src[q]]); }
+        }
     }
+    RNT(6, st);
     return DMRG_OK;
 }
 
@@ -487,10 +528,13 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *o, int32_t max_records, i
     DevBlock L, R;
     int rc = single_site(L, st); if (rc == DMRG_OK) rc = single_site(R, st);
     *n_records = 0;
+    g_tdbg = getenv("DMRG_PLAN_TIMING") != nullptr; g_tl = rn_now(); for (double &v : g_t) v = 0;
     while (rc == DMRG_OK) {
         DevBlock Le, Re;
+        RNT(7, st);
         rc = enlarge(L, 0, o->J, o->Delta, Le, st); if (rc != DMRG_OK) break;                  // line 2
         rc = enlarge(R, 1, o->J, o->Delta, Re, st); if (rc != DMRG_OK) break;
+        RNT(0, st);
         dmrg_problem pr; memset(&pr, 0, sizeof(pr));
         const int32_t target = 0;
         pr.model = DMRG_HEISENBERG; pr.J = o->J; pr.Delta = o->Delta;
@@ -505,14 +549,15 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *o, int32_t max_records, i
         dmrg_handle_t h = nullptr;
         rc = dmrg_plan_create(&pr, &opt, &h); if (rc != DMRG_OK) break;
         Plan *p = reinterpret_cast<Plan *>(h);
+        RNT(1, st);
         DevBuf<double> x; cudaError_t ce = x.alloc((size_t)p->n);
         double lam = 0, rho = 0; int32_t it = 0;
         if (ce != cudaSuccess) { dmrg_plan_destroy(h); return fail(nullptr, DMRG_E_ALLOC, "infinite_heisenberg: eigenvector"); }
         rc = dmrg_lowest_eigenpair(h, nullptr, 1, x.p, &lam, &rho, &it, stream);               // line 3 (start e_argmin(D))
         if (rc == DMRG_NOT_CONVERGED) rc = fail(nullptr, DMRG_E_NUMERIC, "infinite_heisenberg: Davidson did not converge");
+        RNT(2, st);
         double dl = 0, dr = 0; DevBlock Ln, Rn;
-        if (rc == DMRG_OK) rc = renormalise_side(p, Le, 0, x.p, o->m_keep, Ln, &dl, st);       // lines 4-7, left
-        if (rc == DMRG_OK) rc = renormalise_side(p, Re, 1, x.p, o->m_keep, Rn, &dr, st);       // lines 4-7, right
+        if (rc == DMRG_OK) rc = renormalise_both(p, Le, Re, x.p, o->m_keep, Ln, Rn, &dl, &dr, st);      // lines 4-7, both blocks
         const long long n = p->n;
         dmrg_plan_destroy(h);
         if (rc != DMRG_OK) break;
@@ -536,6 +581,7 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *o, int32_t max_records, i
             b.src.swap(bn.src); b.dst.swap(bn.dst); b.ld.swap(bn.ld); b.off.swap(bn.off); std::swap(b.data.p, bn.data.p); std::swap(b.data.n, bn.data.n); std::swap(b.elems, bn.elems);
         }
     }
+    if (g_tdbg) fprintf(stderr, "idmrg ms: enlarge %.1f plan %.1f davidson %.1f alloc %.1f density %.1f sector_eig %.1f select+rotate %.1f other %.1f\n", g_t[0], g_t[1], g_t[2], g_t[3], g_t[4], g_t[5], g_t[6], g_t[7]);
     return rc;
 }
 
