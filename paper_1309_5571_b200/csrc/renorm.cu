@@ -545,7 +545,7 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *o, int32_t max_records, i
         pr.target = &target;
         dmrg_options opt; memset(&opt, 0, sizeof(opt));
         opt.k_max = o->k_max > 0 ? o->k_max : 20; opt.tol = o->tol > 0 ? o->tol : 1e-10; opt.max_iter = o->max_iter > 0 ? o->max_iter : 4000;
-        opt.reorth = 1; opt.seed = 1; opt.check_every = 8;
+        opt.reorth = 1; opt.seed = 1; opt.check_every = 8; opt.reserve_basis = 1;      // (the driver's basis inside the plan's one allocation)
         dmrg_handle_t h = nullptr;
         rc = dmrg_plan_create(&pr, &opt, &h); if (rc != DMRG_OK) break;
         Plan *p = reinterpret_cast<Plan *>(h);
