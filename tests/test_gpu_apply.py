@@ -322,3 +322,40 @@ def test_soak_shapes_multi_rhs_and_streamed_input(lib, monkeypatch):
             assert rel_maxnorm(hw.numpy(), yo) <= HPSI_RTOL, seed
         assert torch.equal(V[0, :lay.n].cpu(), hx)
         plan.close()
+
+
+def test_plan_create_destroy_cycle_leaks_nothing(lib):
+    """A plan is created per superblock (Alg. 1): every device buffer of a plan is a slice of one allocation, freed by
+    dmrg_plan_destroy.  Forty create / apply / destroy cycles over different shapes (both models, with and without a reserved
+    basis, one to three right-hand sides) are run twice: the first pass absorbs what the driver reserves once per process (kernel
+    images, local-memory pool), across the second the free-memory figure must not move; a plan created afterwards still gives
+    the bits of the first one."""
+    import torch
+    p0 = SMALL["cfg2_m160"]()
+    lay0 = rec.Layout(p0)
+    x0 = to_dev(random_vector(lay0.n, 4242))
+    plan = lib.Plan(p0, k_max=8)
+    y_first = plan.apply_H(x0).clone()
+    plan.close()
+    probs = [fuzz_problem(3000 + it, m_max=400) for it in range(40)]
+
+    def cycle():
+        for it, p in enumerate(probs):
+            lay = rec.Layout(p)
+            if lay.n == 0:
+                continue
+            plan = lib.Plan(p, k_max=6, max_rhs=1 + it % 3, reserve_basis=bool(it % 2))
+            y = plan.apply_H(to_dev(random_vector(lay.n, 5000 + it)))
+            assert bool(torch.isfinite(y).all())
+            del y
+            plan.close()
+        torch.cuda.synchronize()
+        torch.cuda.empty_cache()
+        return torch.cuda.mem_get_info()[0]
+
+    free0 = cycle()
+    free1 = cycle()
+    assert abs(free1 - free0) <= (2 << 20), (free0, free1)
+    plan = lib.Plan(p0, k_max=8)
+    assert torch.equal(plan.apply_H(x0), y_first)
+    plan.close()
