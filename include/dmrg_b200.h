@@ -235,7 +235,7 @@ int dmrg_davidson_step_given_w(dmrg_handle_t h, double *V, double *W, int64_t ld
  * cudaHostRegister memory, anything cudaPointerGetAttributes reports as host memory) is not copied
  * by the copy engine at all: loader CTAs of the projection kernel read it over PCIe segment by
  * segment, in the order the work units need the segments, write V(:,k-1) and the operand images,
- * and the other CTAs start on the segments that have arrived (same results bit for bit; a plan of
+ * and the other CTAs start on the 16-row blocks that have arrived (same results bit for bit; a plan of
  * the l-1-1-r strategy and pageable memory take the plain copy).  Always synchronises (stream and
  * side stream) before returning; the other arguments and the return value are those of
  * dmrg_davidson_step.  If the run had already converged the step is a no-op and w_out_host

@@ -116,13 +116,38 @@ __device__ __forceinline__ unsigned smid() {
 struct Producer {
     const double *pP, *pQ;     // the next k-tile's images, bumped by one image per k-tile
     int K, k0;                 // item K; k0 of the next tile to produce
+    int xq_di, xq_dk, xq_rb0;  // streamed x as the Q operand of the item (xq_dk > 0): its k-tiles are row blocks that arrive one by one
 };
+
+// Streamed x: waits until the row blocks [b0, b0 + nb) (nb <= 32) of a segment have arrived (one lane per row block).
+__device__ __forceinline__ void wait_row_blocks(const int *xrb, int rb0, int di, int dk, int b0, int nb, int lane, int *err) {
+    if (lane < nb) {
+        const int b = b0 + lane;
+        const int need = min(BK, di - b * BK) * dk;
+        const int *c = xrb + rb0 + b;
+        long long spins = 0;
+        while (ld_acquire(c) < need) {
+            __nanosleep(64);
+            if (++spins > (1ll << 25)) { atomicExch(err, 1); break; }
+        }
+    }
+    __syncwarp();
+    fence_proxy_async();
+}
 
 __device__ __forceinline__ void begin_item(Producer &pr, const GemmItem *it, double *const *bases, const long long *stride,
                                            int rhs, int n_deps, int m0, int n0, int k0, int lane, const int *ctrl, int *err,
-                                           int xmode) {
-    const int dep = (it->xdep && xmode != 2) ? -1 : it->dep;     // X segments: ready before the first unit unless x is streamed in
-    if (dep >= 0) {            // operand is a T block of this launch (or a streamed X segment): wait until it is all written
+                                           int xmode, const XSeg *xsegs, const int *xrb) {
+    pr.xq_dk = 0;
+    if (it->xdep && xmode == 2) {
+        // streamed x: as the P operand this tile reads rows m0 .. m0 + 63 of the segment (four row blocks, every k-tile: wait
+        // here); as the Q operand its k-tiles ARE the row blocks, in the order of arrival: the stage loop waits for each group
+        const XSeg sg = xsegs[it->dep];
+        if (it->p_base == BASE_XP) wait_row_blocks(xrb, sg.rb0, sg.di, sg.dk, m0 / BK, (min(BM, sg.di - m0) + BK - 1) / BK, lane, err);
+        else { pr.xq_di = sg.di; pr.xq_dk = sg.dk; pr.xq_rb0 = sg.rb0; }
+    }
+    const int dep = it->xdep ? -1 : it->dep;     // X segments: ready before the first unit unless x is streamed in (above)
+    if (dep >= 0) {            // operand is a T block of this launch: wait until it is all written
         if (lane == 0) {
             const int need = it->dep_need;
             const int *c = ctrl + CTRL_DEP0 + rhs * n_deps + dep;
@@ -350,7 +375,8 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     if (xmode == 2 && (int)blockIdx.x < xs.n_loaders) {
         // Streamed input: x lives in pinned host memory.  A few loader CTAs (few, so that the shares arrive over PCIe in the order
         // they were requested) pull it share by share in the order of first use, write the tile images and the device copy,
-        // and publish the elements written per segment; the units' X items wait on those counters (begin_item).  A loader
+        // and publish the elements written per 16-row block of every segment; the units' X items wait for exactly the row blocks they
+        // read next (begin_item, wait_row_blocks).  A loader
         // waits for nothing, and joins the others on the units once the share list is empty.
         __shared__ int s_share;
         for (;;) {
@@ -378,7 +404,13 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             fence_proxy_async();
             __threadfence();
             __syncthreads();
-            if (tid == 0) atomicAdd(&ctrl[CTRL_DEP0 + S.seg], S.hi - S.lo);
+            {   // elements of this share per row block of the segment
+                const int b0 = (S.lo / sg.dk) / BK, b1 = ((S.hi - 1) / sg.dk) / BK;
+                for (int b = b0 + tid; b <= b1; b += THREADS) {
+                    const int lo_b = max(S.lo, b * BK * sg.dk), hi_b = min(S.hi, min((b + 1) * BK, sg.di) * sg.dk);
+                    if (hi_b > lo_b) atomicAdd(&xs.xrb[sg.rb0 + b], hi_b - lo_b);
+                }
+            }
         }
     }
     if (ctr && tid == 0) ctr[1] = globaltimer();
@@ -441,13 +473,14 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 continue;
             }
             Producer pr{};
-            begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, k00, lane, ctrl, err, xmode);
+            begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, k00, lane, ctrl, err, xmode, xsegs, xs.xrb);
             for (int t = 0; t < KT;) {
                 // up to KPS consecutive k-tiles of the current item: their P images are contiguous, and so are their Q images
                 // (a short group comes FIRST: the last stage of an item, and so of the unit, is a full one, which gives the
                 // producer the longest possible cover for its trips to L2 at the boundary)
                 const int rem = min((pr.K - pr.k0 + BK - 1) / BK, KT - t);
                 const int nk = (rem % KPS) ? rem % KPS : KPS;
+                if (pr.xq_dk > 0) wait_row_blocks(xs.xrb, pr.xq_rb0, pr.xq_di, pr.xq_dk, pr.k0 / BK, nk, lane, err);
                 const int s = acquire();
                 StageHdr *h = hdrs + s;
                 const bool last = (t + nk == KT) && !reducer;
@@ -465,7 +498,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
                 g++;
                 if (pr.k0 >= pr.K && t < KT) {
                     p_item++;
-                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, 0, lane, ctrl, err, xmode);
+                    if (p_item < item_count) begin_item(pr, uitems + p_item, s_base, s_stride, rhs, n_deps, m0, n0, 0, lane, ctrl, err, xmode, xsegs, xs.xrb);
                 }
             }
             if (reducer) {
@@ -641,6 +674,7 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
     __syncthreads();
     if (s_is_last) {
         for (int e = tid; e < CTRL_DEP0 + n_deps * nrhs; e += THREADS) ctrl[e] = 0;
+        if (xmode == 2) for (int e = tid; e < xs.n_xrb; e += THREADS) xs.xrb[e] = 0;
     }
 }
 
@@ -684,9 +718,10 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
     XStream xs{};
     const double *x_src = x;
     if (p->x_stream && nrhs == 1 && p->n_xshares > 0) {
-        static const int loaders = []() { const char *e = getenv("DMRG_XLOADERS"); return e ? atoi(e) : 48; }();
+        static const int loaders = []() { const char *e = getenv("DMRG_XLOADERS"); return e ? atoi(e) : 24; }();
         xmode = 2; x_src = p->x_stream;
         xs.shares = p->xshares; xs.n_shares = p->n_xshares; xs.n_loaders = std::max(1, loaders); xs.x_copy = const_cast<double *>(x);
+        xs.xrb = p->xrb; xs.n_xrb = p->n_xrb;
     }
     p->x_stream = nullptr;
     if (nrhs < 1 || nrhs > p->max_rhs) return fail(p, DMRG_E_INVALID_ARG, "apply_H: more right-hand sides than options.max_rhs");

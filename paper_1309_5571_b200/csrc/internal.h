@@ -38,11 +38,13 @@ struct GemmItem {
 };
 
 // Phase 0 table, one entry per segment X_ik (d_i x d_k, row-major at x + seg_off, ascending seg_off): where its P and Q images start
-struct XSeg { long long seg_off, xp_off, xq_off; int di, dk; };
+struct XSeg { long long seg_off, xp_off, xq_off; int di, dk; int rb0, pad; };     // rb0: first of the segment's row-block counters (streamed x)
 // Streamed input (dmrg_davidson_step_host with pinned host memory): a few loader CTAs pull x over PCIe share by share, in
 // the order the units need the segments, and publish the elements written per segment; the other CTAs start on the units.
 struct XShare { int seg, lo, hi, pad; };   // elements [lo, hi) of segment `seg`
-struct XStream { const XShare *shares; int n_shares, n_loaders; double *x_copy; };
+// Row blocks: 16 consecutive rows of a segment X_ik (= one k-tile of its Q images, a quarter of a tile row of its P images); the
+// loaders count the elements written per row block (xrb), and a unit waits for exactly the row blocks its next stage reads.
+struct XStream { const XShare *shares; int n_shares, n_loaders; double *x_copy; int *xrb; int n_xrb; };
 
 struct GemmUnit {
     long long c_off;          // C(0,0) in its base
@@ -153,6 +155,7 @@ struct Plan {
     double *ximg_p = nullptr, *ximg_q = nullptr;   // the input vector as P / Q tile images (rewritten by every apply)
     XSeg *xsegs = nullptr; int n_xsegs = 0;
     XShare *xshares = nullptr; int n_xshares = 0;   // streamed input: shares in the order of first use
+    int *xrb = nullptr; int n_xrb = 0;              // streamed input: elements arrived per row block of every segment
     int n_deps_t = 0;                               // T-block counters; the X-segment counters follow (n_deps = n_deps_t + n_xsegs)
     const double *x_stream = nullptr;               // set for ONE apply_H: device-accessible (pinned host) source of x, streamed
     AxpyItem *axpy = nullptr; int axpy_count = 0;

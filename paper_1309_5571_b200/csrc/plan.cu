@@ -514,12 +514,14 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     // the input vector's segments as tile images (both operand roles), rewritten by phase 0 of every apply
     std::vector<long long> xpOff(P), xqOff(P);
     std::vector<XSeg> xsegs;
+    int n_xrb = 0;
     long long xp_elems = 0, xq_elems = 0;
     for (int op = 0; op < P; op++) {
         const int di = p->dimL[p->pairL[op]], dk = p->dimR[p->pairR[op]];
         xpOff[op] = xp_elems; xp_elems += img_p_elems(di, dk);
         xqOff[op] = xq_elems; xq_elems += img_q_elems(di, dk);
-        xsegs.push_back({p->segOff[op], xpOff[op], xqOff[op], di, dk});
+        xsegs.push_back({p->segOff[op], xpOff[op], xqOff[op], di, dk, n_xrb, 0});
+        n_xrb += (di + BK - 1) / BK;
     }
     for (const Record &r : recs) {
         const int i = p->pairL[r.in_pair], k = p->pairR[r.in_pair];
@@ -719,7 +721,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     items.insert(items.end(), items2.begin(), items2.end());
     p->n_deps_t = (int)tasks1.size();
     p->n_deps = P + p->n_deps_t;
-    // streamed input: shares of <= 3456 elements inside one segment, segments in the order the units first need them
+    // streamed input: shares of <= 3456 elements inside one segment, segments in the order the units first need them; the
+    // loaders count the arrived elements per 16-row block of a segment, the units wait per row block (gemm.cu)
     std::vector<XShare> xshares;
     {
         std::vector<int> first(P, INT_MAX);
@@ -754,6 +757,8 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     CUDA_TRY(p, dev_alloc(p, &p->ximg_q, xq_elems));
     CUDA_TRY(p, dev_alloc(p, &p->xsegs, (long long)xsegs.size()));
     CUDA_TRY(p, dev_alloc(p, &p->xshares, (long long)xshares.size()));
+    p->n_xrb = n_xrb;
+    CUDA_TRY(p, dev_alloc(p, &p->xrb, (long long)n_xrb));
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
@@ -788,6 +793,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     if (!xshares.empty()) CUDA_TRY(p, cudaMemcpy(p->xshares, xshares.data(), xshares.size() * sizeof(XShare), cudaMemcpyHostToDevice));
     if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
     CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
+    CUDA_TRY(p, cudaMemset(p->xrb, 0, sizeof(int) * (size_t)std::max(n_xrb, 1)));
     if (p->trace) CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     CUDA_TRY(p, cudaMemset(p->pool, 0, sizeof(double) * std::max<long long>(bl.pool_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->tws, 0, sizeof(double) * std::max<long long>(tws_elems, 1)));
