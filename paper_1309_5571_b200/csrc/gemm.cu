@@ -746,7 +746,7 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
         if (pf_in && pf_in->base && pf_in->cols > 0 && pf_in->rows > 0) pf = *pf_in;
         const int grid = (int)std::min<long long>((long long)n_units * nrhs, (long long)g_ctas_per_sm * p->sm_count);   // persistent: one wave
         xs.n_loaders = std::min(xs.n_loaders, grid);
-        g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(p->units, p->items, b, p->counters, p->ctrl, n_units,
+        g_variant->fn<<<grid, THREADS, g_variant->smem, st>>>(xmode == 2 ? p->units_stream : p->units, p->items, b, p->counters, p->ctrl, n_units,
                                                               p->n_deps, done_flag, yvec, p->trace, pf, &p->state->gemm_error,
                                                               p->xsegs, p->n_xsegs, x_src, p->n, rh, xmode, p->axpy, xs);
     }

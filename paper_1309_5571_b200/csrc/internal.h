@@ -169,6 +169,7 @@ struct Plan {
     std::vector<std::pair<void **, size_t>> arena_reqs;
     bool own_basis_in_arena = false;
     GemmUnit *units = nullptr;          // ticket order: stage-1 units, then stage-2 units
+    GemmUnit *units_stream = nullptr;   // the same units in the ticket order of a streamed input (plan.cu)
     int n_units1 = 0, n_units2 = 0, n_deps = 0;
     int *ctrl = nullptr;                // Ctrl layout, self-resetting
     unsigned long long *trace = nullptr;   // optional per-unit timeline (4 words per unit), diagnostics

@@ -721,14 +721,62 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     items.insert(items.end(), items2.begin(), items2.end());
     p->n_deps_t = (int)tasks1.size();
     p->n_deps = P + p->n_deps_t;
-    // streamed input: shares of <= 3456 elements inside one segment, segments in the order the units first need them; the
+    // Streamed input (dmrg_davidson_step_host with a pinned v_in): a second copy of the unit list in an order that follows the
+    // arrival of x (ascending address): the stage-1 units sorted by the segment they read (each reads exactly one) and by tile
+    // row, and the stage-2 units of an output `lag` x SM-count tickets after the last stage-1 unit that reads a segment the
+    // output needs.  Same units, tiles, split-K slices and slice order: same bits; waits are on smaller tickets or loaders only.
+    std::vector<GemmUnit> units_s;
+    {
+        static const int s_lag = []() { const char *e = getenv("DMRG_STREAM_LAG"); return e ? atoi(e) : 1; }();
+        std::map<long long, int> op_of_coff;
+        for (const TaskHost &t : tasks2) op_of_coff[t.c_off] = t.out_pair;
+        std::vector<int> key(P, -1);
+        for (const Record &r : recs) key[r.out_pair] = std::max(key[r.out_pair], r.in_pair);
+        std::vector<int> s1;
+        std::vector<std::vector<int>> s2a(P), s2b(P);
+        for (size_t q = 0; q < units.size(); q++) {
+            const GemmUnit &u = units[q];
+            if (u.signal >= 0) { s1.push_back((int)q); continue; }
+            const int o = op_of_coff[u.c_off];
+            if (u.n_split > 1 && u.split_idx == u.n_split - 1) s2b[o].push_back((int)q); else s2a[o].push_back((int)q);
+        }
+        auto seg_of = [&](int q) { return items[units[q].item_begin].dep; };      // a stage-1 unit has one item, and it reads X
+        std::stable_sort(s1.begin(), s1.end(), [&](int a, int b) {
+            if (seg_of(a) != seg_of(b)) return seg_of(a) < seg_of(b);
+            const bool pa = items[units[a].item_begin].p_base == BASE_XP, pb = items[units[b].item_begin].p_base == BASE_XP;
+            const int ra = pa ? units[a].m0 : 1 << 30, rb = pb ? units[b].m0 : 1 << 30;      // P-role tiles by row; Q-role ones need every row
+            return ra < rb;
+        });
+        std::vector<int> oord(P);
+        for (int op = 0; op < P; op++) oord[op] = op;
+        std::stable_sort(oord.begin(), oord.end(), [&](int a, int b) { return key[a] < key[b]; });
+        auto emit2 = [&](int o) { for (int q : s2a[o]) units_s.push_back(units[q]); for (int q : s2b[o]) units_s.push_back(units[q]); };
+        const size_t lag_units = (size_t)std::max(0, s_lag) * (size_t)p->sm_count;
+        std::vector<std::pair<size_t, int>> due;
+        size_t head = 0, oi = 0;
+        for (size_t a = 0; a < s1.size(); a++) {
+            const int sg = seg_of(s1[a]);
+            // outputs whose last segment lies before this unit's: all their stage-1 units are out
+            while (oi < oord.size() && key[oord[oi]] < sg) { due.push_back({units_s.size() + lag_units, oord[oi]}); oi++; }
+            while (head < due.size() && due[head].first <= units_s.size()) emit2(due[head++].second);
+            units_s.push_back(units[s1[a]]);
+        }
+        while (oi < oord.size()) { due.push_back({0, oord[oi]}); oi++; }
+        while (head < due.size()) emit2(due[head++].second);
+        if (units_s.size() != units.size()) return fail(p, DMRG_E_INVALID_ARG, "planner: streamed unit order lost units");
+        for (GemmUnit &u : units_s) u.reducer = 0;
+        std::vector<int> last_of(n_counters, -1);
+        for (size_t q = 0; q < units_s.size(); q++) if (units_s[q].tile_id >= 0) last_of[units_s[q].tile_id] = (int)q;
+        for (int t = 0; t < n_counters; t++) if (last_of[t] >= 0) units_s[last_of[t]].reducer = 1;
+    }
+    // shares of <= 3456 elements inside one segment, segments in the order the units of that list first need them; the
     // loaders count the arrived elements per 16-row block of a segment, the units wait per row block (gemm.cu)
     std::vector<XShare> xshares;
     {
         std::vector<int> first(P, INT_MAX);
-        for (size_t q = 0; q < units.size(); q++)
-            for (int e = 0; e < units[q].item_count; e++) {
-                const GemmItem &it = items[units[q].item_begin + e];
+        for (size_t q = 0; q < units_s.size(); q++)
+            for (int e = 0; e < units_s[q].item_count; e++) {
+                const GemmItem &it = items[units_s[q].item_begin + e];
                 if (it.xdep) first[it.dep] = std::min(first[it.dep], (int)q);
             }
         std::vector<int> ord(P);
@@ -763,6 +811,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
     CUDA_TRY(p, dev_alloc(p, &p->units, (long long)units.size()));
+    CUDA_TRY(p, dev_alloc(p, &p->units_stream, (long long)units_s.size()));
     CUDA_TRY(p, dev_alloc(p, &p->axpy, (long long)axpy.size()));
     CUDA_TRY(p, dev_alloc(p, &p->ctrl, (long long)CTRL_DEP0 + (long long)p->n_deps * R));
     if (getenv("DMRG_TRACE")) {   // diagnostics: per-unit timeline of the last apply (dmrg_get_unit_trace)
@@ -801,6 +850,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     CUDA_TRY(p, cudaMemset(p->D, 0, sizeof(double) * p->n));
     if (!items.empty()) CUDA_TRY(p, cudaMemcpy(p->items, items.data(), items.size() * sizeof(GemmItem), cudaMemcpyHostToDevice));
     if (!units.empty()) CUDA_TRY(p, cudaMemcpy(p->units, units.data(), units.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
+    if (!units_s.empty()) CUDA_TRY(p, cudaMemcpy(p->units_stream, units_s.data(), units_s.size() * sizeof(GemmUnit), cudaMemcpyHostToDevice));
     p->n_units1 = (int)units1.size(); p->n_units2 = (int)units2.size();
     CUDA_TRY(p, cudaMemset(p->state, 0, sizeof(DavState)));
     CUDA_TRY(p, cudaMemset(p->vec_counter, 0, 4 * sizeof(int)));
