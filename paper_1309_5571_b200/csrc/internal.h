@@ -156,6 +156,7 @@ struct Plan {
     XSeg *xsegs = nullptr; int n_xsegs = 0;
     XShare *xshares = nullptr; int n_xshares = 0;   // streamed input: shares in the order of first use
     int *xrb = nullptr; int n_xrb = 0;              // streamed input: elements arrived per row block of every segment
+    int2 *xrows = nullptr; int n_xrows = 0;         // (segment, first row) of every 8-row slab of x: one CTA each in scale_img_rows_kernel
     int n_deps_t = 0;                               // T-block counters; the X-segment counters follow (n_deps = n_deps_t + n_xsegs)
     const double *x_stream = nullptr;               // set for ONE apply_H: device-accessible (pinned host) source of x, streamed
     AxpyItem *axpy = nullptr; int axpy_count = 0;

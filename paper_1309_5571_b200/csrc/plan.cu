@@ -807,6 +807,11 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     CUDA_TRY(p, dev_alloc(p, &p->xshares, (long long)xshares.size()));
     p->n_xrb = n_xrb;
     CUDA_TRY(p, dev_alloc(p, &p->xrb, (long long)n_xrb));
+    std::vector<int2> xrows;
+    for (int op = 0; op < P; op++)
+        if (xsegs[op].dk > 0) for (int r0 = 0; r0 < xsegs[op].di; r0 += 8) xrows.push_back(make_int2(op, r0));
+    p->n_xrows = (int)xrows.size();
+    CUDA_TRY(p, dev_alloc(p, &p->xrows, (long long)xrows.size()));
     CUDA_TRY(p, dev_alloc(p, &p->counters, n_counters));
     CUDA_TRY(p, dev_alloc(p, &p->D, p->n));
     CUDA_TRY(p, dev_alloc(p, &p->items, (long long)items.size()));
@@ -843,6 +848,7 @@ int plan_build(const dmrg_problem *pr, const dmrg_options *opts, Plan **out, con
     if (!axpy.empty()) CUDA_TRY(p, cudaMemcpy(p->axpy, axpy.data(), axpy.size() * sizeof(AxpyItem), cudaMemcpyHostToDevice));
     CUDA_TRY(p, cudaMemset(p->ctrl, 0, sizeof(int) * (CTRL_DEP0 + (size_t)p->n_deps * R)));
     CUDA_TRY(p, cudaMemset(p->xrb, 0, sizeof(int) * (size_t)std::max(n_xrb, 1)));
+    if (!xrows.empty()) CUDA_TRY(p, cudaMemcpy(p->xrows, xrows.data(), xrows.size() * sizeof(int2), cudaMemcpyHostToDevice));
     if (p->trace) CUDA_TRY(p, cudaMemset(p->trace, 0, 32 * (size_t)std::max(p->trace_units, 1)));
     CUDA_TRY(p, cudaMemset(p->pool, 0, sizeof(double) * std::max<long long>(bl.pool_elems, 1)));
     CUDA_TRY(p, cudaMemset(p->tws, 0, sizeof(double) * std::max<long long>(tws_elems, 1)));
