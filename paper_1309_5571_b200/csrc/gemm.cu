@@ -362,6 +362,38 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
             __syncthreads();
             segs = reinterpret_cast<const XSeg *>(smem_raw);
         }
+        if (xs.xrows && segs != xsegs) {
+            // one 8-row slab of a segment per CTA and trip, a warp per row, the lanes along the row: no search and no division per
+            // element, coalesced loads (and Q-image stores); up to eight loads per lane in flight
+            for (int sl = blockIdx.x; sl < xs.n_xrows; sl += gridDim.x) {
+                const int2 rb = xs.xrows[sl];
+                const XSeg sg = segs[rb.x];
+                const int rr = rb.y + warp;
+                if (warp >= 8 || rr >= sg.di) continue;
+                const int dk = sg.dk;
+                const int KTp = (dk + BK - 1) / BK, KTq = (sg.di + BK - 1) / BK;
+                const long long row_off = sg.seg_off + (long long)rr * dk;
+                const long long po = sg.xp_off + (long long)(rr / BM) * KTp * IMG, qo = sg.xq_off + (long long)(rr / BK) * IMG;
+                const int rp = rr % BM, rq = rr % BK;
+                for (int r = 0; r < nrhs; r++) {
+                    const double *xr = x + r * rh.x_ld + row_off;
+                    double *pp = bases.p[BASE_XP] + r * rh.stride[BASE_XP] + po, *pq = bases.p[BASE_XQ] + r * rh.stride[BASE_XQ] + qo;
+                    constexpr int U = 8;
+                    for (int c0 = lane; c0 < dk; c0 += 32 * U) {
+                        double v[U];
+#pragma unroll
+                        for (int q = 0; q < U; q++) { const int c = c0 + 32 * q; v[q] = c < dk ? xr[c] : 0.0; }
+#pragma unroll
+                        for (int q = 0; q < U; q++) {
+                            const int c = c0 + 32 * q;
+                            if (c >= dk) break;
+                            pp[(long long)(c / BK) * IMG + img_p_index(rp, c % BK)] = v[q];
+                            pq[(long long)(c / BN) * KTq * IMG + img_q_index(rq, c % BN)] = v[q];
+                        }
+                    }
+                }
+            }
+        } else
         for (int r = 0; r < nrhs; r++)
             ximg_share(segs, n_xsegs, x + r * rh.x_ld, lo, min(n, lo + share), bases.p[BASE_XP] + r * rh.stride[BASE_XP],
                        bases.p[BASE_XQ] + r * rh.stride[BASE_XQ], tid);
@@ -724,6 +756,10 @@ int apply_H(Plan *p, const double *x, double *y, const int *done_flag, cudaStrea
         xs.xrb = p->xrb; xs.n_xrb = p->n_xrb;
     }
     p->x_stream = nullptr;
+    {
+        static const int p0_rows = []() { const char *e = getenv("DMRG_P0_ROWS"); return e ? atoi(e) : 1; }();
+        if (p0_rows) { xs.xrows = p->xrows; xs.n_xrows = p->n_xrows; }
+    }
     if (nrhs < 1 || nrhs > p->max_rhs) return fail(p, DMRG_E_INVALID_ARG, "apply_H: more right-hand sides than options.max_rhs");
     BasePtrs b;
     b.p[BASE_XP] = p->ximg_p;

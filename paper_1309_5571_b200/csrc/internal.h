@@ -44,7 +44,8 @@ struct XSeg { long long seg_off, xp_off, xq_off; int di, dk; int rb0, pad; };   
 struct XShare { int seg, lo, hi, pad; };   // elements [lo, hi) of segment `seg`
 // Row blocks: 16 consecutive rows of a segment X_ik (= one k-tile of its Q images, a quarter of a tile row of its P images); the
 // loaders count the elements written per row block (xrb), and a unit waits for exactly the row blocks its next stage reads.
-struct XStream { const XShare *shares; int n_shares, n_loaders; double *x_copy; int *xrb; int n_xrb; };
+struct XStream { const XShare *shares; int n_shares, n_loaders; double *x_copy; int *xrb; int n_xrb;
+                 const int2 *xrows; int n_xrows; };      // xrows: (segment, first row) of every 8-row slab of x (phase 0)
 
 struct GemmUnit {
     long long c_off;          // C(0,0) in its base
