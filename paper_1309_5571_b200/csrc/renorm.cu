@@ -188,28 +188,32 @@ sector_eig_kernel(const EigJob *__restrict__ jobs, double *__restrict__ Aall, do
                 s_p[t] = p; s_q[t] = q; s_c[t] = c; s_s[t] = s;
             }
             __syncthreads();
-            // column phase: (A[i][p], A[i][q]) <- (c A[i][p] - s A[i][q], s A[i][p] + c A[i][q]); the same for E
+            // One phase for A' = J^T A J: the rotations of a round act on disjoint index pairs, so A splits into half x half blocks
+            // of 2 x 2 elements (rows of pair t1, columns of pair t2) that are updated independently and in place: columns first,
+            // (x_P, x_Q) <- (c2 x_P - s2 x_Q, s2 x_P + c2 x_Q), then rows, (y_p, y_q) <- (c1 y_p - s1 y_q, s1 y_p + c1 y_q).
+            for (long long e = tid; e < (long long)half * half; e += ET) {
+                const int t1 = (int)(e / half), t2 = (int)(e % half);
+                const double c1 = s_c[t1], s1 = s_s[t1], c2 = s_c[t2], s2 = s_s[t2];
+                if (s1 == 0.0 && s2 == 0.0) continue;
+                const int p = s_p[t1], q = s_q[t1], P = s_p[t2], Q = s_q[t2];
+                const bool hq = q < d, hQ = Q < d;           // (the partner of the odd one out does not exist)
+                double *rp = A + (long long)p * d, *rq = A + (long long)q * d;
+                double apP = rp[P], apQ = hQ ? rp[Q] : 0.0, aqP = hq ? rq[P] : 0.0, aqQ = (hq && hQ) ? rq[Q] : 0.0;
+                const double bpP = c2 * apP - s2 * apQ, bpQ = s2 * apP + c2 * apQ;
+                const double bqP = c2 * aqP - s2 * aqQ, bqQ = s2 * aqP + c2 * aqQ;
+                rp[P] = c1 * bpP - s1 * bqP;
+                if (hQ) rp[Q] = c1 * bpQ - s1 * bqQ;
+                if (hq) { rq[P] = s1 * bpP + c1 * bqP; if (hQ) rq[Q] = s1 * bpQ + c1 * bqQ; }
+            }
+            // E' = E J (columns only), in the same phase
             for (long long e = tid; e < (long long)half * d; e += ET) {
                 const int t = (int)(e % half), i = (int)(e / half);
                 const int p = s_p[t], q = s_q[t];
                 if (q >= d) continue;
                 const double c = s_c[t], s = s_s[t];
                 if (s == 0.0) continue;
-                double *r = A + (long long)i * d; const double ap = r[p], aq = r[q];
-                r[p] = c * ap - s * aq; r[q] = s * ap + c * aq;
                 double *re = E + (long long)i * d; const double ep = re[p], eq = re[q];
                 re[p] = c * ep - s * eq; re[q] = s * ep + c * eq;
-            }
-            __syncthreads();
-            // row phase: (A[p][j], A[q][j]) <- (c A[p][j] - s A[q][j], s A[p][j] + c A[q][j])
-            for (long long e = tid; e < (long long)half * d; e += ET) {
-                const int j = (int)(e % d), t = (int)(e / d);
-                const int p = s_p[t], q = s_q[t];
-                if (q >= d) continue;
-                const double c = s_c[t], s = s_s[t];
-                if (s == 0.0) continue;
-                const double ap = A[(long long)p * d + j], aq = A[(long long)q * d + j];
-                A[(long long)p * d + j] = c * ap - s * aq; A[(long long)q * d + j] = s * ap + c * aq;
             }
             __syncthreads();
         }
