@@ -45,7 +45,8 @@ constexpr int UNIT_WORDS = (int)(sizeof(GemmUnit) / 4);
 static_assert(UNIT_WORDS <= 32, "one lane per word of the unit descriptor");
 
 enum : int { F_DATA = 1, F_LAST = 2, F_EXIT = 4, F_FIRST = 8, F_REDUCE = 16 };
-constexpr int PUBLISH_DELAY = 1;           // stages a consumer warp works on before it fences and signals a finished tile
+constexpr int PUBLISH_DELAY = 1;           // a finished tile is fenced and signalled when the warp turns to its next stage (g + 1); a larger
+                                           // value defers it by whole stages (measured: the waiting units lose what the fence costs here)
 struct StageHdr {
     int flags, ticket, ext_m, ext_n;       // ext: rows / columns of the 64x64 tile that hold data
     int rot, layout, rhs, nk;              // sub-tile rotation and warp layout of the unit (see the consumers); right-hand side; k-tiles in the stage
@@ -603,8 +604,8 @@ grouped_gemm_kernel(const GemmUnit *__restrict__ units, const GemmItem *__restri
         unsigned long long t_start = 0, t_main = 0;
 
         // Deferred publish: a finished tile (a T-block tile, or a parked split-K partial) is announced by this WARP on its
-        // own -- fence, then one atomic per warp; the counters count warps -- and not right after its stores, when the fence
-        // would wait for them to drain, but PUBLISH_DELAY stages into the next unit, or as soon as the warp would block.
+        // own -- fence, then one atomic per warp; the counters count warps -- at the head of a later stage (PUBLISH_DELAY), or as
+        // soon as the warp would block.
         int *pending = nullptr; int pending_g = 0;
         auto flush = [&]() {
             if (pending) {
