@@ -549,7 +549,12 @@ int dmrg_infinite_heisenberg(const dmrg_idmrg_options *o, int32_t max_records, i
         pr.target = &target;
         dmrg_options opt; memset(&opt, 0, sizeof(opt));
         opt.k_max = o->k_max > 0 ? o->k_max : 20; opt.tol = o->tol > 0 ? o->tol : 1e-10; opt.max_iter = o->max_iter > 0 ? o->max_iter : 4000;
-        opt.reorth = 1; opt.seed = 1; opt.check_every = 8; opt.reserve_basis = 1;      // (the driver's basis inside the plan's one allocation)
+        // (reading A16: on a tiny target sector, where k_max is a large fraction of n, ONE Gram-Schmidt pass loses the orthogonality of
+        // the basis and Alg. 3 stalls -- the oracle's textbook Davidson does the same; the first superblocks get the second pass)
+        long long mL = 0, mR = 0;
+        for (int d : Le.dims) mL += d;
+        for (int d : Re.dims) mR += d;
+        opt.reorth = (mL * mR <= 4096) ? 2 : 1; opt.seed = 1; opt.check_every = 8; opt.reserve_basis = 1;      // (the driver's basis inside the plan's one allocation)
         dmrg_handle_t h = nullptr;
         rc = dmrg_plan_create(&pr, &opt, &h); if (rc != DMRG_OK) break;
         Plan *p = reinterpret_cast<Plan *>(h);

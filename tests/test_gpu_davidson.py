@@ -460,3 +460,27 @@ def test_odd_column_stride_takes_the_scalar_path_and_agrees(lib, pad):
         assert abs(lam - ref[i][1]) <= 1e-11 and abs(rho - ref[i][2]) <= 1e-9 + 1e-6 * ref[i][2], (i, lam, ref[i])
     assert float((Va[:ka, :n] - Vb[:kb, :n]).abs().max()) <= 1e-7
     plan.close()
+
+
+@pytest.mark.parametrize("seed", [473, 499])
+def test_tiny_sector_needs_the_second_gram_schmidt_pass(lib, seed):
+    """Reading A16 at its edge: on a tiny target sector (n = 28 / 36 with k_max = 12 / 32) ONE classical Gram-Schmidt pass loses
+    the orthogonality of the basis and Alg. 3 never converges -- in the oracle's textbook Davidson exactly as in the library (this
+    is the algorithm, not the kernels); with reorth = 2 both converge, in the same number of iterations, to the LAPACK value."""
+    import torch
+    p = fuzz_problem(seed, m_max=90)
+    lay = rec.Layout(p)
+    n = lay.n
+    k_max = [6, 12, 20, 32][seed % 4]
+    w = np.linalg.eigvalsh(kron.H_sector(p)[0])
+    D = rec.diag_H(p, lay)
+    apply = oracle_apply(p, lay)
+    x0 = random_vector(n, 31000 + seed)
+    for reorth, expect in ((1, False), (2, True)):
+        ores = odav.davidson_solve(apply, D, x0, k_max, 1e-10, 400, reorth)
+        plan = lib.Plan(p, k_max=k_max, tol=1e-10, max_iter=400, reorth=reorth)
+        rc, lam, x, rho, it = plan.lowest_eigenpair(to_dev(x0))
+        assert ores["converged"] == expect and (rc == lib.DMRG_OK) == expect, (reorth, rc, ores["converged"])
+        if expect:
+            assert it == ores["iters"] and abs(lam - ores["lam"]) <= LAMBDA_ATOL and abs(lam - w[0]) <= LAMBDA_ATOL
+        plan.close()
